@@ -1,0 +1,125 @@
+"""ctypes wrapper around oracle/layup_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  It imports nothing from paper_2410_05985_b200 and the
+product imports nothing from here.  Every function is argument marshalling around
+the C file; the arithmetic of the method (Algorithm 1) lives only
+in layup_oracle.c.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "layup_oracle.c")
+_SO = os.path.join(_HERE, "liblayup_oracle.so")
+_lib = None
+
+
+def build(force=False):
+    """gcc -O2 -ffp-contract=off: no contraction the source does not spell as fmaf()."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        tmp = _SO + ".tmp.%d" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
+                               "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _SO)
+    return _SO
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        c = ctypes
+        _lib.oracle_philox4x32_10.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p]
+        _lib.oracle_philox4x32_10.restype = None
+        _lib.oracle_active.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_float]
+        _lib.oracle_active.restype = c.c_int32
+        _lib.oracle_peer.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_int32, c.c_int32]
+        _lib.oracle_peer.restype = c.c_int32
+        _lib.oracle_schedule.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_int32, c.c_float,
+                                         c.c_void_p, c.c_void_p]
+        _lib.oracle_schedule.restype = None
+        for name, ft in (("oracle_layer_update", c.c_float), ("oracle_layer_update_f64", c.c_double)):
+            f = getattr(_lib, name)
+            f.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
+                          ft, ft, c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_float,
+                          c.c_void_p, c.c_void_p]
+            f.restype = c.c_int
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def philox4x32_10(ctr, key):
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32)
+    key = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.empty(4, dtype=np.uint32)
+    lib().oracle_philox4x32_10(_ptr(ctr), _ptr(key), _ptr(out))
+    return out
+
+
+def active(seed, step, replica, skip_prob):
+    return int(lib().oracle_active(seed, step, replica, skip_prob))
+
+
+def peer(seed, step, layer, replica, K, peer_mode=0):
+    return int(lib().oracle_peer(seed, step, layer, replica, K, peer_mode))
+
+
+def schedule(seed, step, L, K, peer_mode=0, skip_prob=0.0):
+    """-> (peer[L,K] int32 with -1 for inactive replicas, active[K] uint8)."""
+    p = np.empty((L, K), dtype=np.int32)
+    a = np.empty(K, dtype=np.uint8)
+    lib().oracle_schedule(seed, step, L, K, peer_mode, skip_prob, _ptr(p), _ptr(a))
+    return p, a
+
+
+def layer_update(x, g, m, w, lr, mu, seed, step, layer, peer_mode=0, skip_prob=0.0,
+                 peer_in=None, active_in=None):
+    """One (step, layer) in place.  x, g, m: [K, n] (fp32, or x/m fp64 for the shadow); w: [K] fp64."""
+    K, n = x.shape
+    f64 = x.dtype == np.float64
+    assert x.flags.c_contiguous and g.flags.c_contiguous and w.flags.c_contiguous
+    assert g.dtype == np.float32 and g.shape == x.shape and w.dtype == np.float64 and w.shape == (K,)
+    if mu != 0.0:
+        assert m is not None and m.dtype == x.dtype and m.shape == x.shape and m.flags.c_contiguous
+    if peer_in is not None:
+        peer_in = np.ascontiguousarray(peer_in, dtype=np.int32)
+    if active_in is not None:
+        active_in = np.ascontiguousarray(active_in, dtype=np.uint8)
+    f = lib().oracle_layer_update_f64 if f64 else lib().oracle_layer_update
+    rc = f(K, n, _ptr(x), _ptr(g), _ptr(m) if mu != 0.0 else None, _ptr(w), lr, mu, seed, step, layer,
+           peer_mode, skip_prob, _ptr(peer_in), _ptr(active_in))
+    if rc != 0:
+        raise MemoryError("oracle_layer_update failed")
+
+
+class Oracle:
+    """State of K replicas of L layers; round(step, grads) walks the layers L-1 .. 0
+    (output layer first)."""
+
+    def __init__(self, numel, K, lr, momentum=0.0, seed=0, peer_mode=0, skip_prob=0.0, f64=False):
+        self.numel = [int(n) for n in numel]
+        self.L, self.K = len(self.numel), int(K)
+        self.lr, self.mu = lr, momentum
+        self.seed, self.peer_mode, self.skip_prob = int(seed), int(peer_mode), float(skip_prob)
+        self.dt = np.float64 if f64 else np.float32
+        self.x = [np.zeros((self.K, n), dtype=self.dt) for n in self.numel]
+        self.m = [np.zeros((self.K, n), dtype=self.dt) for n in self.numel] if momentum != 0.0 else None
+        self.w = np.full((self.L, self.K), 1.0 / self.K, dtype=np.float64)
+
+    def layer_update(self, step, layer, g):
+        lr = float(np.float32(self.lr)) if self.dt == np.float64 else self.lr
+        mu = float(np.float32(self.mu)) if self.dt == np.float64 else self.mu
+        layer_update(self.x[layer], np.ascontiguousarray(g, dtype=np.float32),
+                     self.m[layer] if self.m is not None else None, self.w[layer],
+                     lr, mu, self.seed, step, layer, self.peer_mode, self.skip_prob)
+
+    def round(self, step, grads):
+        for layer in reversed(range(self.L)):
+            self.layer_update(step, layer, grads[layer])

@@ -1,0 +1,250 @@
+/*
+ * layup_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, single-threaded CPU statement of the LayUp updater step
+ * (arXiv 2410.05985, Algorithm 1 "Updater
+ * Thread i"; weights PAPER.md:106; layer-wise order PAPER.md:23,25,112) for K
+ * workers held as K replicas of every layer.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may call it.  It shares no
+ * code, header, table or constant generator with paper_2410_05985_b200/csrc/.
+ *
+ * The paper's system is racy by design (lock-free overwrites);
+ * the deterministic reading implemented here is the lock-step round of
+ * DESIGN.md "Readings" R1-R10:
+ *
+ *   for one (step t, layer l):
+ *   1. active[i]  : straggler mask, one draw per (t, i)          [PAPER.md:220,229]
+ *   2. peer[i]    : j ~ Random(M-1), never i                     [PAPER.md:101]
+ *      wh[i]      : w_i <- w_i / 2 for a sender                  [PAPER.md:101,106]
+ *   3. local step : x^{i,l} <- x~^{i,l} - eta * grad             [PAPER.md:78,101]
+ *                   (optional heavy-ball momentum, local only; reading R8)
+ *   4. peer update: x^{j,l} <- w_j/(w_i+w_j) x^{j,l} + w_i/(w_i+w_j) x^{i,l}
+ *                   w_j <- w_j + w_i                             [PAPER.md:101]
+ *      applied once per sender of j, ascending sender index, every sender's
+ *      value being its post-local-step, pre-mix value (readings R3, R4).
+ *
+ * Pins (tests/test_oracle_*.py): Philox against cuRAND's library routine run on
+ * the host; worked examples W1/W2 (tests/golden/); mass conservation, weighted-
+ * mean conservation, K=2 exact averaging, convexity, consensus contraction,
+ * brute force over every peer map and mask on tiny layers against a dense
+ * row-stochastic matrix product, K=1 against torch.optim.SGD.
+ * Parity unpinned: the paper's real racy system (no deterministic definition
+ * exists; R3).
+ *
+ * Build: gcc -O2 -ffp-contract=off -shared -fPIC (oracle/__init__.py).  All fp32
+ * multiply-adds that the rule fuses are written as explicit fmaf().
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define TAG_PEER 0u
+#define TAG_SKIP 1u
+#define FIELD_NONE 0xFFFFFFFFu
+
+/* ---- Philox4x32 with 10 rounds (Salmon, Moraes, Dror, Shaw, SC'11) ---------
+ * One round: two 32x32->64 products of counter words 0 and 2 with the two
+ * multipliers; new counter = (hi1^c1^k0, lo1, hi0^c3^k1, lo0); the key is
+ * bumped by the two Weyl constants between rounds.                          */
+static void philox_round(uint32_t c[4], const uint32_t k[2]) {
+  const uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c[0];
+  const uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c[2];
+  const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+  const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+  const uint32_t n0 = hi1 ^ c[1] ^ k[0];
+  const uint32_t n2 = hi0 ^ c[3] ^ k[1];
+  c[0] = n0; c[1] = lo1; c[2] = n2; c[3] = lo0;
+}
+
+void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c[4] = {ctr[0], ctr[1], ctr[2], ctr[3]};
+  uint32_t k[2] = {key[0], key[1]};
+  for (int r = 0; r < 10; ++r) {
+    if (r > 0) { k[0] += 0x9E3779B9u; k[1] += 0xBB67AE85u; }
+    philox_round(c, k);
+  }
+  out[0] = c[0]; out[1] = c[1]; out[2] = c[2]; out[3] = c[3];
+}
+
+/* first output word for key = seed, counter = (c0,c1,c2,c3) */
+static uint32_t draw(uint64_t seed, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
+  const uint32_t ctr[4] = {c0, c1, c2, c3};
+  const uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)};
+  uint32_t out[4];
+  oracle_philox4x32_10(ctr, key, out);
+  return out[0];
+}
+
+/* Reading R10: one skip draw per (step, replica); the layer field is unused so a
+ * straggler idles for the whole round.  Threshold computed in
+ * double from the fp32 probability, clamped to 2^32-1.                        */
+int32_t oracle_active(uint64_t seed, int64_t step, int32_t replica, float skip_prob) {
+  if (!(skip_prob > 0.0f)) return 1;
+  double th = (double)skip_prob * 4294967296.0;
+  if (th > 4294967295.0) th = 4294967295.0;
+  const uint32_t thr = (uint32_t)th;
+  const uint32_t r = draw(seed, (uint32_t)step, FIELD_NONE, (uint32_t)replica, TAG_SKIP);
+  return r < thr ? 0 : 1;
+}
+
+/* PAPER.md:101 "j ~ Random(M-1)": uniform over the K-1 other workers (R5).
+ * uint32 -> [0, K-2] by multiply-high (R6), then skip over self.
+ * peer_mode 0: a fresh peer per (step, layer, replica) (BASELINE.json north_star)
+ * peer_mode 1: one peer per (step, replica), shared by all layers (Alg. 1).   */
+int32_t oracle_peer(uint64_t seed, int64_t step, int32_t layer, int32_t replica,
+                    int32_t K, int32_t peer_mode) {
+  if (K < 2) return -1;
+  const uint32_t lf = peer_mode == 0 ? (uint32_t)layer : FIELD_NONE;
+  const uint32_t r = draw(seed, (uint32_t)step, lf, (uint32_t)replica, TAG_PEER);
+  const uint32_t q = (uint32_t)(((uint64_t)r * (uint64_t)(K - 1)) >> 32);
+  return (int32_t)(q + (q >= (uint32_t)replica ? 1u : 0u));
+}
+
+/* peer[l*K+i] = chosen peer, or -1 when replica i is inactive (or K == 1). */
+void oracle_schedule(uint64_t seed, int64_t step, int32_t L, int32_t K, int32_t peer_mode,
+                     float skip_prob, int32_t *peer, uint8_t *active) {
+  for (int32_t i = 0; i < K; ++i) active[i] = (uint8_t)oracle_active(seed, step, i, skip_prob);
+  for (int32_t l = 0; l < L; ++l)
+    for (int32_t i = 0; i < K; ++i)
+      peer[(size_t)l * K + i] = active[i] ? oracle_peer(seed, step, l, i, K, peer_mode) : -1;
+}
+
+/* ---- one (step, layer) of the updater, fp32 state, fp64 push-sum weights ----
+ * x, g, m : [K][n] row-major fp32 (m may be NULL when mu == 0);  w : [K] fp64.
+ * peer_in/active_in: if non-NULL the schedule is taken from them instead of
+ * being drawn (used by the brute-force tests to enumerate every schedule).
+ * Returns 0, or -1 on allocation failure.                                    */
+int oracle_layer_update(int32_t K, int64_t n, float *x, const float *g, float *m, double *w,
+                        float lr, float mu, uint64_t seed, int64_t step, int32_t layer,
+                        int32_t peer_mode, float skip_prob,
+                        const int32_t *peer_in, const uint8_t *active_in) {
+  int32_t *peer = (int32_t *)malloc(sizeof(int32_t) * (size_t)K);
+  uint8_t *active = (uint8_t *)malloc((size_t)K);
+  double *wh = (double *)malloc(sizeof(double) * (size_t)K);
+  float *y = (float *)malloc(sizeof(float) * (size_t)K * (size_t)(n > 0 ? n : 1));
+  float *acc = (float *)malloc(sizeof(float) * (size_t)(n > 0 ? n : 1));
+  if (!peer || !active || !wh || !y || !acc) {
+    free(peer); free(active); free(wh); free(y); free(acc);
+    return -1;
+  }
+
+  /* 1. straggler mask; 2. peer choice and weight halving */
+  for (int32_t i = 0; i < K; ++i) {
+    active[i] = active_in ? active_in[i] : (uint8_t)oracle_active(seed, step, i, skip_prob);
+    if (active[i] && K >= 2) {
+      peer[i] = peer_in ? peer_in[i] : oracle_peer(seed, step, layer, i, K, peer_mode);
+      wh[i] = w[i] * 0.5;
+    } else {
+      peer[i] = -1;          /* inactive (or alone): no push, weight not halved */
+      wh[i] = w[i];
+    }
+  }
+
+  /* 3. local step on the current copy */
+  for (int32_t i = 0; i < K; ++i) {
+    float *xi = x + (size_t)i * n;
+    const float *gi = g + (size_t)i * n;
+    float *yi = y + (size_t)i * n;
+    if (active[i]) {
+      if (mu != 0.0f) {
+        float *mi = m + (size_t)i * n;
+        for (int64_t e = 0; e < n; ++e) {
+          const float mm = fmaf(mu, mi[e], gi[e]);   /* m <- mu*m + g        */
+          mi[e] = mm;
+          yi[e] = fmaf(-lr, mm, xi[e]);              /* y  = x - eta*m       */
+        }
+      } else {
+        for (int64_t e = 0; e < n; ++e) yi[e] = fmaf(-lr, gi[e], xi[e]);   /* y = x - eta*g */
+      }
+    } else {
+      for (int64_t e = 0; e < n; ++e) yi[e] = xi[e];
+    }
+  }
+
+  /* 4. peer update, once per sender of j in ascending sender index */
+  for (int32_t j = 0; j < K; ++j) {
+    double W = wh[j];
+    const float *yj = y + (size_t)j * n;
+    for (int64_t e = 0; e < n; ++e) acc[e] = yj[e];
+    for (int32_t i = 0; i < K; ++i) {
+      if (!(active[i] && peer[i] == j)) continue;
+      const float alpha = (float)(wh[i] / (W + wh[i]));   /* w_i/(w_i+w_j), one rounding */
+      const float *yi = y + (size_t)i * n;
+      for (int64_t e = 0; e < n; ++e) {
+        const float d = yi[e] - acc[e];
+        acc[e] = fmaf(alpha, d, acc[e]);                  /* = (1-a)*x_j + a*x_i */
+      }
+      W = W + wh[i];                                      /* w_j <- w_j + w_i    */
+    }
+    float *xj = x + (size_t)j * n;
+    for (int64_t e = 0; e < n; ++e) xj[e] = acc[e];
+    w[j] = W;
+  }
+
+  free(peer); free(active); free(wh); free(y); free(acc);
+  return 0;
+}
+
+/* ---- fp64 shadow: same schedule, every value in double, and the mix written in
+ * its closed form  x_j <- (wh_j y_j + sum_i wh_i y_i) / (wh_j + sum_i wh_i)
+ * (PAPER.md:101 applied once per sender telescopes to this weighted centroid).
+ * Used for the 100-round error bound and as an independent statement of step 4. */
+int oracle_layer_update_f64(int32_t K, int64_t n, double *x, const float *g, double *m, double *w,
+                            double lr, double mu, uint64_t seed, int64_t step, int32_t layer,
+                            int32_t peer_mode, float skip_prob,
+                            const int32_t *peer_in, const uint8_t *active_in) {
+  int32_t *peer = (int32_t *)malloc(sizeof(int32_t) * (size_t)K);
+  uint8_t *active = (uint8_t *)malloc((size_t)K);
+  double *wh = (double *)malloc(sizeof(double) * (size_t)K);
+  double *y = (double *)malloc(sizeof(double) * (size_t)K * (size_t)(n > 0 ? n : 1));
+  if (!peer || !active || !wh || !y) {
+    free(peer); free(active); free(wh); free(y);
+    return -1;
+  }
+  for (int32_t i = 0; i < K; ++i) {
+    active[i] = active_in ? active_in[i] : (uint8_t)oracle_active(seed, step, i, skip_prob);
+    if (active[i] && K >= 2) {
+      peer[i] = peer_in ? peer_in[i] : oracle_peer(seed, step, layer, i, K, peer_mode);
+      wh[i] = w[i] * 0.5;
+    } else {
+      peer[i] = -1;
+      wh[i] = w[i];
+    }
+  }
+  for (int32_t i = 0; i < K; ++i) {
+    for (int64_t e = 0; e < n; ++e) {
+      const size_t o = (size_t)i * n + e;
+      if (active[i]) {
+        if (mu != 0.0) {
+          m[o] = mu * m[o] + (double)g[o];
+          y[o] = x[o] - lr * m[o];
+        } else {
+          y[o] = x[o] - lr * (double)g[o];
+        }
+      } else {
+        y[o] = x[o];
+      }
+    }
+  }
+  for (int32_t j = 0; j < K; ++j) {
+    double W = wh[j];
+    for (int32_t i = 0; i < K; ++i)
+      if (active[i] && peer[i] == j) W += wh[i];
+    for (int64_t e = 0; e < n; ++e) {
+      double s = wh[j] * y[(size_t)j * n + e];
+      for (int32_t i = 0; i < K; ++i)
+        if (active[i] && peer[i] == j) s += wh[i] * y[(size_t)i * n + e];
+      x[(size_t)j * n + e] = s / W;
+    }
+  }
+  /* weights are updated after all receivers are done (wh is the pre-round view) */
+  for (int32_t j = 0; j < K; ++j) {
+    double W = wh[j];
+    for (int32_t i = 0; i < K; ++i)
+      if (active[i] && peer[i] == j) W = W + wh[i];
+    w[j] = W;
+  }
+  free(peer); free(active); free(wh); free(y);
+  return 0;
+}
