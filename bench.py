@@ -1,0 +1,356 @@
+#!/usr/bin/env python
+"""bench.py -- param-updates/s and effective HBM GB/s of the LayUp update+gossip round.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl ours|reference]
+
+A "step" is one layup_round(): the whole hot path (straggler mask, peer choice, push-sum
+weights, local step, push, peer mix, reverse-layer work list) over all K replicas of all
+layers of one synthetic batch of gradients.  Default workload = BASELINE.json:configs[2]
+(K=16 replicas of the GPT-2-medium parameter set, fp32 + momentum), the largest config
+and the one north_star's bandwidth target is stated on.
+
+Prints ONE JSON line.  N > 1 (torchrun): the path does not shard (north_star: "no
+sharding across GPUs, no collectives"), so each rank runs an independent replica set
+("replicas only") and value is the sum over ranks / max time.
+--impl reference times the CPU oracle as it stands on a bounded sample of the workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+import torch  # noqa: E402
+
+import synth  # noqa: E402
+
+METRIC = "param_updates_per_s"
+UNIT = "param-updates/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="gpt2m_k16")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--mode", default="round", choices=["round", "layers"],
+                    help="round: one persistent launch per step; layers: L per-layer launches on 4 streams")
+    return ap.parse_args()
+
+
+def get_workload(name):
+    try:
+        return synth.workload(int(name))
+    except ValueError:
+        return synth.workload(name)
+
+
+def bytes_per_update(w):
+    return 20 if w.momentum != 0.0 else 12
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def committed_traffic(name):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(name)
+        except Exception:
+            pass
+    return None
+
+
+# ---- oracle sample (cpu_baseline and --impl reference) -------------------------------
+def oracle_sample(w, seconds, steps=None, warmup=0):
+    """Times oracle/ as it stands, single-threaded, on a bounded sample of the workload:
+    the LAST layers of the layer list (output side first, as the path walks them) up to a
+    budget of parameter updates per round."""
+    import oracle
+    budget = 200e6                       # param-updates per round in the sample
+    layers, tot = [], 0
+    for l in reversed(range(w.L)):
+        if layers and tot + w.K * w.numel[l] > budget:
+            break
+        layers.append(l)
+        tot += w.K * w.numel[l]
+    layers = sorted(layers)
+    sub = synth.shrink(w, [w.numel[l] for l in layers])
+    ref = oracle.Oracle(sub.numel, sub.K, sub.lr, sub.momentum, sub.seed, sub.peer_mode, sub.skip_prob)
+    xs, grads_fn = synth.host_state(sub)
+    for l in range(sub.L):
+        ref.x[l][:] = xs[l]
+    grads = grads_fn(0)
+    for s in range(warmup):
+        ref.round(s, grads)
+    done, t_used, step = 0, 0.0, warmup
+    per_step_updates = []
+    while True:
+        _, act = oracle.schedule(sub.seed, step, sub.L, sub.K, sub.peer_mode, sub.skip_prob)
+        t0 = time.perf_counter()
+        ref.round(step, grads)
+        t_used += time.perf_counter() - t0
+        per_step_updates.append(int(act.sum()) * sum(sub.numel))
+        step += 1
+        done += 1
+        if steps is not None:
+            if done >= steps:
+                break
+        elif t_used >= seconds or done >= 50:
+            break
+    ups = sum(per_step_updates) / t_used
+    sample = "layers %d..%d of %d (%.1fM params/replica, K=%d), %d rounds, single thread" % (
+        layers[0], layers[-1], w.L, sum(sub.numel) / 1e6, sub.K, done)
+    return ups, t_used / done, sample, sum(per_step_updates) / done
+
+
+def run_reference(args, w, rank, world):
+    if rank != 0:
+        return
+    ups, s_per_step, sample, _ = oracle_sample(w, args.cpu_seconds, steps=args.steps, warmup=min(args.warmup, 1))
+    line = {
+        "metric": METRIC, "value": ups, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": s_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic", "impl": "reference",
+        "config": {"workload": "%s (%s)" % (w.name, w.note), "K": w.K, "L": w.L,
+                   "params_per_replica": w.params_per_replica, "momentum": w.momentum},
+        "cpu_baseline": {"value": ups, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": ups, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---- clocks sampling ------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def summary(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1] or [r for (_, r) in self.rows[-3:]]
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); smax = float(f[1])
+            except Exception:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def algorithmic_bytes(w, lu, steps_range):
+    """12/20 B per active param-update, 8 B for an idle replica that receives."""
+    if w.skip_prob == 0.0:
+        n = w.K * w.params_per_replica
+        return [bytes_per_update(w) * n] * len(steps_range), [n] * len(steps_range)
+    bts, ups = [], []
+    numel = np.array(w.numel, dtype=np.float64)
+    for s in steps_range:
+        peer, active = lu.layup_schedule(s)
+        b = u = 0.0
+        for i in range(w.K):
+            if active[i]:
+                b += bytes_per_update(w) * numel.sum(); u += numel.sum()
+            else:
+                recv = np.array([(peer[l] == i).any() for l in range(w.L)])
+                b += 8 * numel[recv].sum()
+        bts.append(b); ups.append(u)
+    return bts, ups
+
+
+def run_ours(args, w, rank, world, local_rank):
+    from paper_2410_05985_b200 import WHAT_G, WHAT_X, LayUp
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    lu = LayUp(w.K, w.numel, w.lr, w.momentum, w.seed + 1000 * rank, w.peer_mode, w.skip_prob, device=local_rank)
+    for l in range(w.L):
+        synth.fill_init_(w, l, lu.view(WHAT_X, l))
+        synth.fill_grad_(w, 0, l, lu.view(WHAT_G, l), data_seed=w.seed + 1000 * rank)
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream() for _ in range(4)] if args.mode == "layers" else None
+
+    def one_step(s):
+        if args.mode == "round":
+            lu.layup_round(s)
+        else:
+            for k, l in enumerate(reversed(range(w.L))):
+                lu.layup_layer_update(s, l, streams[k % 4])
+
+    step = 0
+    for _ in range(args.warmup):
+        one_step(step); step += 1
+    lu.layup_sync()
+    launches0 = lu.layup_launch_count()
+    lu.layup_profile(True)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    time.sleep(0.3)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.perf_counter()
+    first = step
+    if streams:
+        for st in streams:
+            st.wait_stream(torch.cuda.current_stream())
+    ev0.record()
+    for _ in range(args.steps):
+        one_step(step); step += 1
+    if streams:
+        for st in streams:
+            torch.cuda.current_stream().wait_stream(st)
+    ev1.record()
+    barrier()
+    t1 = time.perf_counter()
+    ms = ev0.elapsed_time(ev1)
+    n_k, k_ms = lu.layup_profile_read()
+    lu.layup_profile(False)
+    launches = lu.layup_launch_count() - launches0
+    clocks = sampler.summary(t0, t1) if sampler else None
+    bts, ups = algorithmic_bytes(w, lu, range(first, first + args.steps))
+
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        tot = torch.tensor([sum(ups), sum(bts)], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        job_updates, job_bytes = float(tot[0].item()), float(tot[1].item())
+    else:
+        job_updates, job_bytes = float(sum(ups)), float(sum(bts))
+    value = job_updates / (ms * 1e-3)
+    eff_gbs = job_bytes / (ms * 1e-3) / 1e9
+
+    # ---- roofline of the dominant kernel (the fused update kernel), this rank
+    peak, peak_src = measured_peak()
+    k_avg_ms = k_ms / max(n_k, 1)
+    bytes_per_launch = sum(bts) / max(n_k, 1)
+    achieved = bytes_per_launch / (k_avg_ms * 1e-3) / 1e9 if k_avg_ms > 0 else 0.0
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": committed_traffic(w.name), "kernel": "layup_update_kernel",
+                "kernel_ms_avg": k_avg_ms, "kernel_launches": n_k, "algorithmic_bytes_per_launch": bytes_per_launch,
+                "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0}
+
+    # ---- e2e: same metric through the C-ABI with HOST buffers (h2d grads + d2h params in the timed region)
+    e2e = None
+    if not args.no_e2e:
+        try:
+            total = w.K * w.params_per_replica
+            g_host = torch.empty(total, dtype=torch.float32, pin_memory=True)
+            x_host = torch.empty(total, dtype=torch.float32, pin_memory=True)
+            off = 0
+            for l, n in enumerate(w.numel):      # host gradients = the same synthetic batch, unpadded
+                g_host[off:off + w.K * n].view(w.K, n).copy_(lu.view(WHAT_G, l))
+                off += w.K * n
+            torch.cuda.synchronize()
+            lu.layup_round_host(step, g_host, x_host); step += 1       # warm-up (stream/event creation)
+            barrier()
+            te0 = time.perf_counter()
+            e_first = step
+            for _ in range(args.e2e_steps):
+                lu.layup_round_host(step, g_host, x_host); step += 1
+            barrier()
+            e_s = time.perf_counter() - te0
+            if dist is not None:
+                t = torch.tensor([e_s], device="cuda", dtype=torch.float64)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                e_s = float(t.item())
+            _, e_ups = algorithmic_bytes(w, lu, range(e_first, e_first + args.e2e_steps))
+            e2e = {"value": world * sum(e_ups) / e_s, "unit": UNIT, "h2d_bytes_per_step": 4 * total,
+                   "d2h_bytes_per_step": 4 * total, "steps": args.e2e_steps, "ms_per_step": e_s / args.e2e_steps * 1e3,
+                   "api": "layup_round_host (pinned host grads in, params out, layer-pipelined)"}
+            del g_host, x_host
+        except Exception as ex:                  # e.g. the box cannot pin 2 x K x N x 4 bytes
+            e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
+    lu.layup_sync()
+
+    if rank != 0:
+        return
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        c_ups, _, sample, _ = oracle_sample(w, args.cpu_seconds)
+        cpu = {"value": c_ups, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+               "host_cores": os.cpu_count()}
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "%s (%s)" % (w.name, w.note), "K": w.K, "L": w.L,
+                   "params_per_replica": w.params_per_replica, "momentum": w.momentum, "lr": w.lr,
+                   "skip_prob": w.skip_prob, "mode": args.mode, "parallelism": "replicas only x%d" % world,
+                   "l2": "inputs larger than L2" if job_bytes / args.steps / world > 4 * 126e6 else
+                         "L2-resident working set (launch-latency bound, see DESIGN.md)"},
+        "effective_hbm_gbs": eff_gbs, "frac_of_8TBs_nominal": eff_gbs / world / 8000.0,
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    w = get_workload(args.config)
+    if args.impl == "reference":
+        run_reference(args, w, rank, world)
+    else:
+        run_ours(args, w, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

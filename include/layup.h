@@ -1,0 +1,143 @@
+/*
+ * layup.h -- C-ABI boundary of the B200-native LayUp hot path.
+ *
+ * What the library computes: the "Updater Thread i" of Algorithm 1 of LayUp
+ * (arXiv 2410.05985) for K workers held as K fp32
+ * replicas of every layer in ONE device arena:  per layer, as soon as its gradient
+ * exists, the local SGD step on each worker's copy
+ * ("Local Update"), then the push-sum gossip mix of that copy into a
+ * randomly chosen peer's copy of the same layer ("Peer Update",
+ * PAPER.md:104-106 weights), with no buffer or queue.  The
+ * deterministic reading of the paper's racy system is DESIGN.md "Readings" R1-R17.
+ *
+ * Conventions
+ *  - All functions return int: LAYUP_OK (0) or a negative LAYUP_E* code; no exceptions,
+ *    no abort, nothing printed.  layup_last_error() gives the text of the last failure.
+ *  - Pointers are HOST pointers unless the comment says DEVICE.
+ *  - Launching calls (layup_layer_update, layup_round) are ASYNCHRONOUS on the given
+ *    CUDA stream; device-side failures surface at layup_sync().
+ *  - Ownership: the caller allocates the arena (device memory) and the streams and keeps
+ *    them alive until layup_destroy(); the library borrows them.  It owns only its small
+ *    tables (layer table, schedule tables, weights w[L][K]); it never allocates
+ *    parameter-sized memory ("without buffering").
+ *  - A ctx is used from one host thread at a time.
+ *  - There is no CPU fallback: without a CUDA device every launching call fails with
+ *    LAYUP_ECUDA.
+ *
+ * Arena layout (DEVICE, fp32): three sections X | G | M (M only if momentum != 0), each
+ * `section_floats` long.  Inside a section layers are stored in order 0..L-1; layer l
+ * holds its K replicas back to back, each slice padded to a multiple of 32 floats
+ * (128 B):   addr(what, i, l, e) = arena + what*section + base[l] + i*pad[l] + e.
+ * The arena base must be 128-byte aligned.  layup_init() zeroes the whole arena, so the
+ * pads are zero and stay zero; fill x (and g before every step) through layup_ptr().
+ */
+#ifndef LAYUP_H_
+#define LAYUP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LAYUP_OK      0
+#define LAYUP_EINVAL -1   /* bad argument, misaligned or too-small arena              */
+#define LAYUP_ESTATE -2   /* (step, layer) applied out of order or twice              */
+#define LAYUP_ECUDA  -3   /* CUDA failure (no device, launch or runtime error)        */
+
+#define LAYUP_WHAT_X 0    /* parameters x^{i,l}                 */
+#define LAYUP_WHAT_G 1    /* gradient of this step   ("Backward pass")    */
+#define LAYUP_WHAT_M 2    /* momentum buffer, local to the worker (R8)      */
+
+#define LAYUP_MAX_K 1024  /* replicas (workers) per ctx                               */
+
+typedef struct layup_ctx layup_ctx;   /* opaque */
+
+typedef struct {
+  int32_t  K;          /* workers M of the paper, 1 <= K <= LAYUP_MAX_K    */
+  int32_t  L;          /* layers                                                          */
+  const int64_t *numel;/* [L] HOST: elements per layer (unpadded), each >= 1              */
+  float    lr;         /* eta                                               */
+  float    momentum;   /* mu; 0 => no M section in the arena                              */
+  uint64_t seed;       /* Philox key of the peer selector and of the straggler mask       */
+  int32_t  peer_mode;  /* 0: peer per (step, layer, replica)  [BASELINE.json north_star]
+                          1: peer per (step, replica), all layers [Alg. 1, PAPER.md:101,453] */
+  float    skip_prob;  /* straggler mode: P(replica idles this round); 0 = off            */
+  int32_t  device;     /* CUDA ordinal                                                    */
+} layup_config;
+
+/* Bytes of device memory the arena needs for this config (X + G (+ M), padded). Pure. */
+int layup_arena_bytes(const layup_config *cfg, size_t *bytes);
+
+/* Create a ctx over a caller-owned DEVICE arena (128-B aligned, >= layup_arena_bytes).
+ * Zeroes the arena, sets w[l][i] = 1/K and the step counters to 0.
+ * Synchronous. */
+int layup_init(const layup_config *cfg, void *arena_dev, size_t arena_bytes, layup_ctx **out);
+
+/* Waits for the ctx's pending work, frees the library's tables.  The arena is untouched. */
+int layup_destroy(layup_ctx *ctx);
+
+/* Borrowed DEVICE pointer to slice (what, replica, layer) and its unpadded length. */
+int layup_ptr(layup_ctx *ctx, int32_t what, int32_t replica, int32_t layer,
+              float **dptr, int64_t *numel);
+
+/* Learning-rate schedules live outside the path: lr is a scalar that
+ * the next launching call picks up. */
+int layup_set_lr(layup_ctx *ctx, float lr);
+
+/* The paper's per-layer event ("Notify" / "Wait for notification"):
+ * for ALL K replicas of `layer`, round `step`: straggler mask, peer choice, weight
+ * halving, local step, push, peer update, weight add.  The layer's gradients must
+ * already be in the arena in `cuda_stream` order.  Each layer must see step = 0,1,2,...
+ * exactly once each (LAYUP_ESTATE otherwise); layers may be issued in any order and on
+ * any streams -- they are independent -- but the paper's order is L-1 first
+ * (PAPER.md:23,25).  cuda_stream: a cudaStream_t (NULL = legacy default stream). */
+int layup_layer_update(layup_ctx *ctx, int64_t step, int32_t layer, void *cuda_stream);
+
+/* All layers L-1 .. 0 of round `step` in one persistent grouped launch that drains a
+ * reverse-layer-ordered work list.  Bit-identical to L calls of layup_layer_update. */
+int layup_round(layup_ctx *ctx, int64_t step, void *cuda_stream);
+
+/* layup_round with HOST buffers, layer-pipelined: for l = L-1..0 copy layer l's
+ * gradients host->device, update it, copy its new parameters device->host, the three
+ * stages of consecutive layers overlapping on the library's own streams.
+ * g_host, x_host: [sum_l K*numel[l]] fp32, layer-major then replica (no padding), should
+ * be pinned for the copies to be asynchronous; x_host may be NULL (no read-back).
+ * Returns after the last copy has completed (synchronous). */
+int layup_round_host(layup_ctx *ctx, int64_t step, const float *g_host, float *x_host);
+
+/* Wait for every stream the ctx has launched on; report the first sticky CUDA error. */
+int layup_sync(layup_ctx *ctx);
+
+/* ---- introspection for parity (read-only) ---------------------------------------- */
+
+/* Host-side pure function: the peer replica `replica` pushes to in (step, layer), as
+ * the kernels draw it: Philox4x32-10, key = seed, counter = (step, layer, replica, 0);
+ * pass layer = -1 for peer_mode 1.  K >= 2. */
+int layup_peer(uint64_t seed, int64_t step, int32_t layer, int32_t replica, int32_t K,
+               int32_t *peer);
+
+/* Runs the DEVICE schedule stage for round `step` without touching any state and copies
+ * it out: peer[l*K+i] (-1 if replica i is inactive) and active[i].  Synchronous. */
+int layup_schedule(layup_ctx *ctx, int64_t step, int32_t *peer /*[L*K]*/, uint8_t *active /*[K]*/);
+
+/* Current push-sum weights w[l*K+i], after all work issued so far. */
+int layup_weights(layup_ctx *ctx, double *w /*[L*K]*/);
+
+/* Device time of the fused update kernel, measured with CUDA events on the launch
+ * stream: enable, run, layup_sync(), read (and reset).  launches = update-kernel
+ * launches timed, total_ms = sum of their durations. */
+int layup_profile(layup_ctx *ctx, int32_t enable);
+int layup_profile_read(layup_ctx *ctx, int64_t *launches, double *total_ms);
+
+/* Kernels launched by this ctx so far (schedule + update kernels). */
+int layup_launch_count(layup_ctx *ctx, int64_t *launches);
+
+/* Text of the last error on this ctx (ctx may be NULL: last error of a ctx-less call). */
+const char *layup_last_error(layup_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LAYUP_H_ */

@@ -1,0 +1,201 @@
+"""ctypes binding of include/layup.h -- argument marshalling only.
+
+Every step of the path runs in the kernels of csrc/*.cu.  torch is used for device
+memory (the arena is a torch uint8 tensor) and streams; nothing here computes.  If
+csrc/liblayup.so is missing or no CUDA device is present, calls fail loudly.
+"""
+import ctypes
+import os
+from typing import List, Optional, Sequence
+
+import numpy as np
+import torch
+
+LAYUP_OK, LAYUP_EINVAL, LAYUP_ESTATE, LAYUP_ECUDA = 0, -1, -2, -3
+WHAT_X, WHAT_G, WHAT_M = 0, 1, 2
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "csrc", "liblayup.so")
+_lib = None
+
+
+class LayUpError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("layup error %d: %s" % (code, text))
+        self.code = code
+
+
+class _Config(ctypes.Structure):
+    _fields_ = [("K", ctypes.c_int32), ("L", ctypes.c_int32), ("numel", ctypes.POINTER(ctypes.c_int64)),
+                ("lr", ctypes.c_float), ("momentum", ctypes.c_float), ("seed", ctypes.c_uint64),
+                ("peer_mode", ctypes.c_int32), ("skip_prob", ctypes.c_float), ("device", ctypes.c_int32)]
+
+
+EXPORTS = ["layup_arena_bytes", "layup_init", "layup_destroy", "layup_ptr", "layup_set_lr",
+           "layup_layer_update", "layup_round", "layup_round_host", "layup_sync", "layup_peer",
+           "layup_schedule", "layup_weights", "layup_profile", "layup_profile_read", "layup_launch_count",
+           "layup_last_error"]
+
+
+def load_library():
+    """dlopen csrc/liblayup.so (built by __graft_entry__.build()); no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        raise LayUpError(LAYUP_ECUDA, "%s not built: run `python -c 'import __graft_entry__ as g; g.build()'`" % _SO)
+    lib = ctypes.CDLL(_SO)
+    c = ctypes
+    vp, i32, i64 = c.c_void_p, c.c_int32, c.c_int64
+    sig = {
+        "layup_arena_bytes": [c.POINTER(_Config), c.POINTER(c.c_size_t)],
+        "layup_init": [c.POINTER(_Config), vp, c.c_size_t, c.POINTER(vp)],
+        "layup_destroy": [vp],
+        "layup_ptr": [vp, i32, i32, i32, c.POINTER(vp), c.POINTER(i64)],
+        "layup_set_lr": [vp, c.c_float],
+        "layup_layer_update": [vp, i64, i32, vp],
+        "layup_round": [vp, i64, vp],
+        "layup_round_host": [vp, i64, vp, vp],
+        "layup_sync": [vp],
+        "layup_peer": [c.c_uint64, i64, i32, i32, i32, c.POINTER(i32)],
+        "layup_schedule": [vp, i64, vp, vp],
+        "layup_weights": [vp, vp],
+        "layup_profile": [vp, i32],
+        "layup_profile_read": [vp, c.POINTER(i64), c.POINTER(c.c_double)],
+        "layup_launch_count": [vp, c.POINTER(i64)],
+    }
+    for name, args in sig.items():
+        f = getattr(lib, name)
+        f.argtypes, f.restype = args, c.c_int
+    lib.layup_last_error.argtypes, lib.layup_last_error.restype = [vp], c.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc, ctx=None):
+    if rc != LAYUP_OK:
+        raise LayUpError(rc, (load_library().layup_last_error(ctx) or b"").decode())
+
+
+def _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device):
+    arr = (ctypes.c_int64 * len(numel))(*[int(n) for n in numel])
+    cfg = _Config(int(K), len(numel), arr, float(lr), float(momentum), int(seed), int(peer_mode),
+                  float(skip_prob), int(device))
+    cfg._keep = arr
+    return cfg
+
+
+def layup_arena_bytes(K, numel, momentum=0.0) -> int:
+    out = ctypes.c_size_t(0)
+    cfg = _config(K, numel, 0.0, momentum, 0, 0, 0.0, 0)
+    _check(load_library().layup_arena_bytes(ctypes.byref(cfg), ctypes.byref(out)))
+    return out.value
+
+
+def layup_peer(seed, step, layer, replica, K) -> int:
+    out = ctypes.c_int32(0)
+    _check(load_library().layup_peer(int(seed), int(step), int(layer), int(replica), int(K), ctypes.byref(out)))
+    return out.value
+
+
+def _stream_handle(stream) -> Optional[int]:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream or None
+    if isinstance(stream, torch.cuda.Stream):
+        return stream.cuda_stream or None
+    return int(stream) or None
+
+
+class LayUp:
+    """One ctx = K replicas of L layers in one torch-allocated arena on one GPU."""
+
+    def __init__(self, K: int, numel: Sequence[int], lr: float, momentum: float = 0.0, seed: int = 0,
+                 peer_mode: int = 0, skip_prob: float = 0.0, device: int = 0):
+        self.lib = load_library()
+        self.K, self.L, self.numel = int(K), len(numel), [int(n) for n in numel]
+        self.momentum = float(momentum)
+        self.device = torch.device("cuda", device)
+        self._cfg = _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device)
+        nbytes = ctypes.c_size_t(0)
+        _check(self.lib.layup_arena_bytes(ctypes.byref(self._cfg), ctypes.byref(nbytes)))
+        self.arena_bytes = nbytes.value
+        if not torch.cuda.is_available():
+            raise LayUpError(LAYUP_ECUDA, "no CUDA device: the LayUp path has no CPU fallback")
+        self.arena = torch.empty(self.arena_bytes + 128, dtype=torch.uint8, device=self.device)
+        shift = (-self.arena.data_ptr()) % 128
+        self._arena_f32 = self.arena[shift:shift + self.arena_bytes].view(torch.float32)
+        torch.cuda.synchronize(self.device)
+        ctx = ctypes.c_void_p()
+        _check(self.lib.layup_init(ctypes.byref(self._cfg), self._arena_f32.data_ptr(), self.arena_bytes,
+                                   ctypes.byref(ctx)))
+        self.ctx = ctx
+        self._base = self._arena_f32.data_ptr()
+
+    # -- arena views (torch plumbing: a view is a slice of the arena tensor) --------------
+    def ptr(self, what: int, replica: int, layer: int):
+        p, n = ctypes.c_void_p(), ctypes.c_int64()
+        _check(self.lib.layup_ptr(self.ctx, what, replica, layer, ctypes.byref(p), ctypes.byref(n)), self.ctx)
+        return p.value, n.value
+
+    def view(self, what: int, layer: int) -> torch.Tensor:
+        """[K, numel] fp32 strided view of all replicas of one layer."""
+        p0, n = self.ptr(what, 0, layer)
+        off0 = (p0 - self._base) // 4
+        if self.K > 1:
+            p1, _ = self.ptr(what, 1, layer)
+            stride = (p1 - p0) // 4
+        else:
+            stride = (n + 31) // 32 * 32
+        return self._arena_f32.as_strided((self.K, n), (stride, 1), off0)
+
+    # -- the C-ABI calls, same names -----------------------------------------------------
+    def layup_set_lr(self, lr: float):
+        _check(self.lib.layup_set_lr(self.ctx, lr), self.ctx)
+
+    def layup_layer_update(self, step: int, layer: int, stream=None):
+        _check(self.lib.layup_layer_update(self.ctx, step, layer, _stream_handle(stream)), self.ctx)
+
+    def layup_round(self, step: int, stream=None):
+        _check(self.lib.layup_round(self.ctx, step, _stream_handle(stream)), self.ctx)
+
+    def layup_round_host(self, step: int, g_host: torch.Tensor, x_host: Optional[torch.Tensor]):
+        _check(self.lib.layup_round_host(self.ctx, step, g_host.data_ptr(),
+                                         x_host.data_ptr() if x_host is not None else None), self.ctx)
+
+    def layup_sync(self):
+        _check(self.lib.layup_sync(self.ctx), self.ctx)
+
+    def layup_schedule(self, step: int):
+        peer = np.empty((self.L, self.K), dtype=np.int32)
+        active = np.empty(self.K, dtype=np.uint8)
+        _check(self.lib.layup_schedule(self.ctx, step, peer.ctypes.data, active.ctypes.data), self.ctx)
+        return peer, active
+
+    def layup_weights(self) -> np.ndarray:
+        w = np.empty((self.L, self.K), dtype=np.float64)
+        _check(self.lib.layup_weights(self.ctx, w.ctypes.data), self.ctx)
+        return w
+
+    def layup_profile(self, enable: bool):
+        _check(self.lib.layup_profile(self.ctx, 1 if enable else 0), self.ctx)
+
+    def layup_profile_read(self):
+        n, ms = ctypes.c_int64(), ctypes.c_double()
+        _check(self.lib.layup_profile_read(self.ctx, ctypes.byref(n), ctypes.byref(ms)), self.ctx)
+        return n.value, ms.value
+
+    def layup_launch_count(self) -> int:
+        n = ctypes.c_int64()
+        _check(self.lib.layup_launch_count(self.ctx, ctypes.byref(n)), self.ctx)
+        return n.value
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            self.lib.layup_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

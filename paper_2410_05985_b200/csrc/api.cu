@@ -1,0 +1,406 @@
+// C-ABI of liblayup (include/layup.h): argument checking, arena layout, step bookkeeping,
+// launches.  Every step of the path itself runs in the kernels of schedule.cu / update.cu.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/layup.h"
+#include "layup_internal.cuh"
+#include "philox.cuh"
+
+using namespace layup;
+
+struct layup_ctx {
+  int32_t K = 0, L = 0, device = 0, peer_mode = 0;
+  float lr = 0.f, mu = 0.f, skip_prob = 0.f;
+  uint32_t skip_thr = 0;
+  uint64_t seed = 0;
+  std::vector<LayerDesc> layers;          // host copy
+  std::vector<long long> tile_prefix;     // host copy, by position (pos p = layer L-1-p)
+  std::vector<int64_t> next_step;         // per layer
+  long long section = 0;                  // floats per section
+  float *arena = nullptr;
+  int C = 0, log2C = 0, smem = 0, ctas_per_sm = 1, n_sm = 1;
+  // device tables
+  LayerDesc *d_layers = nullptr;
+  long long *d_tile_prefix = nullptr;
+  double *d_w = nullptr;
+  SchedTables t{};
+  int32_t *d_peer_scratch = nullptr;
+  unsigned char *d_active_scratch = nullptr;
+  // bookkeeping
+  std::vector<cudaStream_t> streams;      // every stream launched on
+  cudaStream_t own_stream = nullptr;      // introspection / init
+  cudaStream_t s_h2d = nullptr, s_cmp = nullptr, s_d2h = nullptr;
+  std::vector<cudaEvent_t> ev_h2d, ev_done;
+  bool profiling = false;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pending, prof_pool;
+  int64_t launches = 0;
+  std::string err;
+};
+
+static thread_local std::string g_err;
+
+static int fail(layup_ctx *ctx, int code, const char *fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (ctx) ctx->err = buf;
+  g_err = buf;
+  return code;
+}
+
+#define CU_TRY(ctx, expr)                                                                      \
+  do {                                                                                         \
+    cudaError_t e__ = (expr);                                                                  \
+    if (e__ != cudaSuccess)                                                                    \
+      return fail(ctx, LAYUP_ECUDA, "%s: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+  } while (0)
+
+static long long pad32(long long n) { return (n + 31) / 32 * 32; }
+
+static int check_config(const layup_config *cfg) {
+  if (!cfg) return fail(nullptr, LAYUP_EINVAL, "config is NULL");
+  if (cfg->K < 1 || cfg->K > LAYUP_MAX_K) return fail(nullptr, LAYUP_EINVAL, "K=%d outside [1,%d]", cfg->K, LAYUP_MAX_K);
+  if (cfg->L < 1 || !cfg->numel) return fail(nullptr, LAYUP_EINVAL, "L=%d / numel invalid", cfg->L);
+  for (int l = 0; l < cfg->L; ++l)
+    if (cfg->numel[l] < 1) return fail(nullptr, LAYUP_EINVAL, "numel[%d]=%lld < 1", l, (long long)cfg->numel[l]);
+  if (!(cfg->skip_prob >= 0.f && cfg->skip_prob <= 1.f)) return fail(nullptr, LAYUP_EINVAL, "skip_prob outside [0,1]");
+  if (cfg->peer_mode != 0 && cfg->peer_mode != 1) return fail(nullptr, LAYUP_EINVAL, "peer_mode must be 0 or 1");
+  if (!(cfg->momentum >= 0.f) || !(cfg->lr == cfg->lr)) return fail(nullptr, LAYUP_EINVAL, "lr / momentum invalid");
+  return LAYUP_OK;
+}
+
+static long long section_floats(const layup_config *cfg) {
+  long long s = 0;
+  for (int l = 0; l < cfg->L; ++l) s += (long long)cfg->K * pad32(cfg->numel[l]);
+  return s;
+}
+
+extern "C" int layup_arena_bytes(const layup_config *cfg, size_t *bytes) {
+  int rc = check_config(cfg);
+  if (rc) return rc;
+  if (!bytes) return fail(nullptr, LAYUP_EINVAL, "bytes is NULL");
+  *bytes = (size_t)section_floats(cfg) * sizeof(float) * (cfg->momentum != 0.f ? 3 : 2);
+  return LAYUP_OK;
+}
+
+static void note_stream(layup_ctx *ctx, cudaStream_t s) {
+  if (std::find(ctx->streams.begin(), ctx->streams.end(), s) == ctx->streams.end()) ctx->streams.push_back(s);
+}
+
+static int env_int(const char *name, int dflt) {
+  const char *v = getenv(name);
+  return v && *v ? atoi(v) : dflt;
+}
+
+extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena_bytes, layup_ctx **out) {
+  int rc = check_config(cfg);
+  if (rc) return rc;
+  if (!out) return fail(nullptr, LAYUP_EINVAL, "out is NULL");
+  *out = nullptr;
+  size_t need = 0;
+  layup_arena_bytes(cfg, &need);
+  if (!arena_dev || ((uintptr_t)arena_dev & 127u)) return fail(nullptr, LAYUP_EINVAL, "arena NULL or not 128-byte aligned");
+  if (arena_bytes < need) return fail(nullptr, LAYUP_EINVAL, "arena too small: %zu < %zu", arena_bytes, need);
+
+  int ndev = 0;
+  CU_TRY(nullptr, cudaGetDeviceCount(&ndev));
+  if (cfg->device < 0 || cfg->device >= ndev) return fail(nullptr, LAYUP_EINVAL, "device %d of %d", cfg->device, ndev);
+  CU_TRY(nullptr, cudaSetDevice(cfg->device));
+
+  layup_ctx *ctx = new layup_ctx();
+  ctx->K = cfg->K; ctx->L = cfg->L; ctx->device = cfg->device; ctx->peer_mode = cfg->peer_mode;
+  ctx->lr = cfg->lr; ctx->mu = cfg->momentum; ctx->skip_prob = cfg->skip_prob; ctx->seed = cfg->seed;
+  {
+    double th = (double)cfg->skip_prob * 4294967296.0;     // DESIGN R10: threshold in double, clamped
+    if (th > 4294967295.0) th = 4294967295.0;
+    ctx->skip_thr = cfg->skip_prob > 0.f ? (uint32_t)th : 0u;
+  }
+  ctx->arena = (float *)arena_dev;
+  ctx->section = section_floats(cfg);
+
+  // tile shape: C float4 columns per replica, K*C items per tile
+  const int items_target = std::max(256, env_int("LAYUP_TILE_ITEMS", 1024));
+  int C = 8;
+  while ((long long)cfg->K * C * 2 <= items_target && C < 4096) C *= 2;
+  ctx->C = C;
+  ctx->log2C = 0;
+  while ((1 << ctx->log2C) < C) ++ctx->log2C;
+  ctx->smem = (int)update_smem_bytes(cfg->K, C);
+
+  const int K = cfg->K, L = cfg->L;
+  ctx->layers.resize(L);
+  long long base = 0;
+  for (int l = 0; l < L; ++l) {
+    ctx->layers[l] = LayerDesc{base, pad32(cfg->numel[l]), cfg->numel[l]};
+    base += (long long)K * ctx->layers[l].pad;
+  }
+  ctx->tile_prefix.assign(L + 1, 0);
+  for (int p = 0; p < L; ++p) {
+    const LayerDesc &d = ctx->layers[L - 1 - p];
+    const long long cols = d.pad / 4;
+    ctx->tile_prefix[p + 1] = ctx->tile_prefix[p] + (cols + C - 1) / C;
+  }
+  ctx->next_step.assign(L, 0);
+
+  cudaDeviceProp prop;
+  auto bail = [&](int code) { layup_destroy(ctx); return code; };
+#define CU_TRY_INIT(expr)                                                                               \
+  do {                                                                                                  \
+    cudaError_t e__ = (expr);                                                                           \
+    if (e__ != cudaSuccess) {                                                                           \
+      fail(nullptr, LAYUP_ECUDA, "%s: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+      return bail(LAYUP_ECUDA);                                                                         \
+    }                                                                                                   \
+  } while (0)
+  CU_TRY_INIT(cudaGetDeviceProperties(&prop, cfg->device));
+  ctx->n_sm = prop.multiProcessorCount;
+  if ((size_t)ctx->smem > prop.sharedMemPerBlockOptin) {
+    fail(nullptr, LAYUP_EINVAL, "K=%d needs %d B of shared memory per CTA", K, ctx->smem);
+    return bail(LAYUP_EINVAL);
+  }
+  CU_TRY_INIT(update_kernel_setup(ctx->smem, &ctx->ctas_per_sm));
+  if (ctx->ctas_per_sm < 1) ctx->ctas_per_sm = 1;
+  const int cap = env_int("LAYUP_CTAS_PER_SM", 0);
+  if (cap > 0 && cap < ctx->ctas_per_sm) ctx->ctas_per_sm = cap;
+
+  CU_TRY_INIT(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+  CU_TRY_INIT(cudaMalloc(&ctx->d_layers, sizeof(LayerDesc) * L));
+  CU_TRY_INIT(cudaMalloc(&ctx->d_tile_prefix, sizeof(long long) * (L + 1)));
+  CU_TRY_INIT(cudaMalloc(&ctx->d_w, sizeof(double) * L * K));
+  CU_TRY_INIT(cudaMalloc(&ctx->t.peer, sizeof(int32_t) * L * K));
+  CU_TRY_INIT(cudaMalloc(&ctx->t.recv_off, sizeof(int32_t) * L * (K + 1)));
+  CU_TRY_INIT(cudaMalloc(&ctx->t.senders, sizeof(int32_t) * L * K));
+  CU_TRY_INIT(cudaMalloc(&ctx->t.alpha, sizeof(float) * L * K));
+  CU_TRY_INIT(cudaMalloc(&ctx->t.flags, (size_t)L * K));
+  CU_TRY_INIT(cudaMalloc(&ctx->d_peer_scratch, sizeof(int32_t) * L * K));
+  CU_TRY_INIT(cudaMalloc(&ctx->d_active_scratch, (size_t)K));
+  CU_TRY_INIT(cudaMemcpy(ctx->d_layers, ctx->layers.data(), sizeof(LayerDesc) * L, cudaMemcpyHostToDevice));
+  CU_TRY_INIT(cudaMemcpy(ctx->d_tile_prefix, ctx->tile_prefix.data(), sizeof(long long) * (L + 1), cudaMemcpyHostToDevice));
+  std::vector<double> w0((size_t)L * K, 1.0 / (double)K);              // PAPER.md:106  w_i = 1/M
+  CU_TRY_INIT(cudaMemcpy(ctx->d_w, w0.data(), sizeof(double) * L * K, cudaMemcpyHostToDevice));
+  CU_TRY_INIT(cudaMemset(ctx->t.recv_off, 0, sizeof(int32_t) * L * (K + 1)));
+  CU_TRY_INIT(cudaMemset(ctx->t.flags, 0, (size_t)L * K));
+  CU_TRY_INIT(cudaMemset(arena_dev, 0, need));                          // pads are zero and stay zero
+  CU_TRY_INIT(cudaDeviceSynchronize());
+#undef CU_TRY_INIT
+  *out = ctx;
+  return LAYUP_OK;
+}
+
+extern "C" int layup_destroy(layup_ctx *ctx) {
+  if (!ctx) return LAYUP_OK;
+  cudaSetDevice(ctx->device);
+  for (cudaStream_t s : ctx->streams) cudaStreamSynchronize(s);
+  for (cudaStream_t s : {ctx->own_stream, ctx->s_h2d, ctx->s_cmp, ctx->s_d2h})
+    if (s) { cudaStreamSynchronize(s); cudaStreamDestroy(s); }
+  for (auto &v : {ctx->ev_h2d, ctx->ev_done})
+    for (cudaEvent_t e : v) cudaEventDestroy(e);
+  for (auto &pr : ctx->prof_pending) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+  for (auto &pr : ctx->prof_pool) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+  cudaFree(ctx->d_layers); cudaFree(ctx->d_tile_prefix); cudaFree(ctx->d_w);
+  cudaFree(ctx->t.peer); cudaFree(ctx->t.recv_off); cudaFree(ctx->t.senders); cudaFree(ctx->t.alpha);
+  cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_active_scratch);
+  delete ctx;
+  return LAYUP_OK;
+}
+
+extern "C" int layup_ptr(layup_ctx *ctx, int32_t what, int32_t replica, int32_t layer, float **dptr, int64_t *numel) {
+  if (!ctx || !dptr) return fail(ctx, LAYUP_EINVAL, "ctx or dptr is NULL");
+  if (what < 0 || what > 2 || (what == LAYUP_WHAT_M && ctx->mu == 0.f)) return fail(ctx, LAYUP_EINVAL, "what=%d not in this arena", what);
+  if (replica < 0 || replica >= ctx->K || layer < 0 || layer >= ctx->L) return fail(ctx, LAYUP_EINVAL, "replica %d / layer %d out of range", replica, layer);
+  const LayerDesc &d = ctx->layers[layer];
+  *dptr = ctx->arena + (long long)what * ctx->section + d.base + (long long)replica * d.pad;
+  if (numel) *numel = d.numel;
+  return LAYUP_OK;
+}
+
+extern "C" int layup_set_lr(layup_ctx *ctx, float lr) {
+  if (!ctx || !(lr == lr)) return fail(ctx, LAYUP_EINVAL, "ctx NULL or lr NaN");
+  ctx->lr = lr;
+  return LAYUP_OK;
+}
+
+// schedule kernel + update kernel for positions [pos_begin, pos_end) of the reverse-ordered list
+static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaStream_t s) {
+  const int L = ctx->L;
+  SchedParams sp{};
+  sp.t = ctx->t; sp.w = ctx->d_w; sp.seed = ctx->seed; sp.step = (uint32_t)step; sp.skip_thr = ctx->skip_thr;
+  sp.K = ctx->K; sp.L = L; sp.peer_mode = ctx->peer_mode;
+  sp.layer_begin = L - pos_end;                       // layers [L-pos_end, L-pos_begin)
+  CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
+
+  UpdateParams up{};
+  up.x = ctx->arena;
+  up.g = ctx->arena + ctx->section;
+  up.m = ctx->mu != 0.f ? ctx->arena + 2 * ctx->section : nullptr;
+  up.layers = ctx->d_layers; up.tile_prefix = ctx->d_tile_prefix; up.t = ctx->t;
+  up.tile_begin = ctx->tile_prefix[pos_begin]; up.tile_end = ctx->tile_prefix[pos_end];
+  up.K = ctx->K; up.L = L; up.C = ctx->C; up.log2C = ctx->log2C; up.pos_begin = pos_begin;
+  up.neg_lr = -ctx->lr; up.mu = ctx->mu;
+  const long long tiles = up.tile_end - up.tile_begin;
+  const int grid = (int)std::min<long long>(tiles, (long long)ctx->n_sm * ctx->ctas_per_sm);
+
+  std::pair<cudaEvent_t, cudaEvent_t> ev{nullptr, nullptr};
+  if (ctx->profiling) {
+    if (!ctx->prof_pool.empty()) { ev = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
+    else { CU_TRY(ctx, cudaEventCreate(&ev.first)); CU_TRY(ctx, cudaEventCreate(&ev.second)); }
+    CU_TRY(ctx, cudaEventRecord(ev.first, s));
+  }
+  CU_TRY(ctx, launch_update(up, grid, ctx->smem, s));
+  if (ctx->profiling) {
+    CU_TRY(ctx, cudaEventRecord(ev.second, s));
+    ctx->prof_pending.push_back(ev);
+  }
+  ctx->launches += 2;
+  note_stream(ctx, s);
+  return LAYUP_OK;
+}
+
+extern "C" int layup_layer_update(layup_ctx *ctx, int64_t step, int32_t layer, void *cuda_stream) {
+  if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
+  if (layer < 0 || layer >= ctx->L) return fail(ctx, LAYUP_EINVAL, "layer %d out of range", layer);
+  if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
+  if (ctx->next_step[layer] != step)
+    return fail(ctx, LAYUP_ESTATE, "layer %d expects step %lld, got %lld", layer, (long long)ctx->next_step[layer], (long long)step);
+  CU_TRY(ctx, cudaSetDevice(ctx->device));
+  const int pos = ctx->L - 1 - layer;
+  int rc = issue(ctx, step, pos, pos + 1, (cudaStream_t)cuda_stream);
+  if (rc == LAYUP_OK) ctx->next_step[layer] = step + 1;
+  return rc;
+}
+
+extern "C" int layup_round(layup_ctx *ctx, int64_t step, void *cuda_stream) {
+  if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
+  if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
+  for (int l = 0; l < ctx->L; ++l)
+    if (ctx->next_step[l] != step)
+      return fail(ctx, LAYUP_ESTATE, "layer %d expects step %lld, got %lld", l, (long long)ctx->next_step[l], (long long)step);
+  CU_TRY(ctx, cudaSetDevice(ctx->device));
+  int rc = issue(ctx, step, 0, ctx->L, (cudaStream_t)cuda_stream);
+  if (rc == LAYUP_OK)
+    for (int l = 0; l < ctx->L; ++l) ctx->next_step[l] = step + 1;
+  return rc;
+}
+
+extern "C" int layup_round_host(layup_ctx *ctx, int64_t step, const float *g_host, float *x_host) {
+  if (!ctx || !g_host) return fail(ctx, LAYUP_EINVAL, "ctx or g_host is NULL");
+  if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
+  const int L = ctx->L, K = ctx->K;
+  for (int l = 0; l < L; ++l)
+    if (ctx->next_step[l] != step)
+      return fail(ctx, LAYUP_ESTATE, "layer %d expects step %lld, got %lld", l, (long long)ctx->next_step[l], (long long)step);
+  CU_TRY(ctx, cudaSetDevice(ctx->device));
+  if (!ctx->s_h2d) {
+    CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
+    CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->s_cmp, cudaStreamNonBlocking));
+    CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
+    ctx->ev_h2d.resize(L); ctx->ev_done.resize(L);
+    for (int l = 0; l < L; ++l) {
+      CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->ev_h2d[l], cudaEventDisableTiming));
+      CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->ev_done[l], cudaEventDisableTiming));
+    }
+  }
+  std::vector<long long> hoff(L + 1, 0);                   // host offsets, layer-major, unpadded
+  for (int l = 0; l < L; ++l) hoff[l + 1] = hoff[l] + (long long)K * ctx->layers[l].numel;
+  float *gsec = ctx->arena + ctx->section;
+  for (int l = L - 1; l >= 0; --l) {                       // output layer first
+    const LayerDesc &d = ctx->layers[l];
+    const size_t row = (size_t)d.numel * sizeof(float);
+    CU_TRY(ctx, cudaMemcpy2DAsync(gsec + d.base, (size_t)d.pad * sizeof(float), g_host + hoff[l], row, row, K,
+                                  cudaMemcpyHostToDevice, ctx->s_h2d));
+    CU_TRY(ctx, cudaEventRecord(ctx->ev_h2d[l], ctx->s_h2d));
+    CU_TRY(ctx, cudaStreamWaitEvent(ctx->s_cmp, ctx->ev_h2d[l], 0));
+    const int pos = L - 1 - l;
+    int rc = issue(ctx, step, pos, pos + 1, ctx->s_cmp);
+    if (rc) return rc;
+    ctx->next_step[l] = step + 1;
+    if (x_host) {
+      CU_TRY(ctx, cudaEventRecord(ctx->ev_done[l], ctx->s_cmp));
+      CU_TRY(ctx, cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_done[l], 0));
+      CU_TRY(ctx, cudaMemcpy2DAsync(x_host + hoff[l], row, ctx->arena + d.base, (size_t)d.pad * sizeof(float), row, K,
+                                    cudaMemcpyDeviceToHost, ctx->s_d2h));
+    }
+  }
+  CU_TRY(ctx, cudaStreamSynchronize(ctx->s_h2d));
+  CU_TRY(ctx, cudaStreamSynchronize(ctx->s_cmp));
+  CU_TRY(ctx, cudaStreamSynchronize(ctx->s_d2h));
+  return LAYUP_OK;
+}
+
+extern "C" int layup_sync(layup_ctx *ctx) {
+  if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
+  CU_TRY(ctx, cudaSetDevice(ctx->device));
+  for (cudaStream_t s : ctx->streams) CU_TRY(ctx, cudaStreamSynchronize(s));
+  CU_TRY(ctx, cudaGetLastError());
+  return LAYUP_OK;
+}
+
+extern "C" int layup_peer(uint64_t seed, int64_t step, int32_t layer, int32_t replica, int32_t K, int32_t *peer) {
+  if (!peer || K < 2 || replica < 0 || replica >= K || layer < -1) return fail(nullptr, LAYUP_EINVAL, "layup_peer: bad argument");
+  *peer = draw_peer(seed, (uint32_t)step, layer < 0 ? kNoLayer : (uint32_t)layer, replica, K);
+  return LAYUP_OK;
+}
+
+extern "C" int layup_schedule(layup_ctx *ctx, int64_t step, int32_t *peer, uint8_t *active) {
+  if (!ctx || !peer || !active) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
+  CU_TRY(ctx, cudaSetDevice(ctx->device));
+  CU_TRY(ctx, launch_peers_only(ctx->seed, (uint32_t)step, ctx->skip_thr, ctx->K, ctx->L, ctx->peer_mode,
+                                ctx->d_peer_scratch, ctx->d_active_scratch, ctx->own_stream));
+  ctx->launches += 1;
+  CU_TRY(ctx, cudaMemcpyAsync(peer, ctx->d_peer_scratch, sizeof(int32_t) * ctx->L * ctx->K, cudaMemcpyDeviceToHost, ctx->own_stream));
+  CU_TRY(ctx, cudaMemcpyAsync(active, ctx->d_active_scratch, (size_t)ctx->K, cudaMemcpyDeviceToHost, ctx->own_stream));
+  CU_TRY(ctx, cudaStreamSynchronize(ctx->own_stream));
+  return LAYUP_OK;
+}
+
+extern "C" int layup_weights(layup_ctx *ctx, double *w) {
+  if (!ctx || !w) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  int rc = layup_sync(ctx);
+  if (rc) return rc;
+  CU_TRY(ctx, cudaMemcpy(w, ctx->d_w, sizeof(double) * ctx->L * ctx->K, cudaMemcpyDeviceToHost));
+  return LAYUP_OK;
+}
+
+extern "C" int layup_profile(layup_ctx *ctx, int32_t enable) {
+  if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
+  ctx->profiling = enable != 0;
+  return LAYUP_OK;
+}
+
+extern "C" int layup_profile_read(layup_ctx *ctx, int64_t *launches, double *total_ms) {
+  if (!ctx || !launches || !total_ms) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  int rc = layup_sync(ctx);
+  if (rc) return rc;
+  double tot = 0.0;
+  for (auto &pr : ctx->prof_pending) {
+    float ms = 0.f;
+    CU_TRY(ctx, cudaEventElapsedTime(&ms, pr.first, pr.second));
+    tot += ms;
+  }
+  *launches = (int64_t)ctx->prof_pending.size();
+  *total_ms = tot;
+  ctx->prof_pool.insert(ctx->prof_pool.end(), ctx->prof_pending.begin(), ctx->prof_pending.end());
+  ctx->prof_pending.clear();
+  return LAYUP_OK;
+}
+
+extern "C" int layup_launch_count(layup_ctx *ctx, int64_t *launches) {
+  if (!ctx || !launches) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  *launches = ctx->launches;
+  return LAYUP_OK;
+}
+
+extern "C" const char *layup_last_error(layup_ctx *ctx) {
+  return ctx ? ctx->err.c_str() : g_err.c_str();
+}

@@ -1,0 +1,60 @@
+// Internal declarations shared by the library's translation units (not part of the C-ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace layup {
+
+constexpr int kThreads = 256;          // threads per CTA of the update kernel
+constexpr int kFlagActive = 1;         // replica takes its local step and pushes this round
+constexpr int kFlagRecv = 2;           // replica receives at least one push this round
+
+// One (replica-major) layer of the arena; offsets in floats inside a section.
+struct LayerDesc {
+  long long base;      // offset of replica 0's slice
+  long long pad;       // slice stride (numel rounded up to 32 floats = 128 B)
+  long long numel;     // unpadded elements
+};
+
+// Per-(layer) schedule tables, written by the schedule kernel, read by the update kernel.
+struct SchedTables {
+  int32_t *peer;            // [L*K]   chosen peer or -1
+  int32_t *recv_off;        // [L*(K+1)] CSR by receiver
+  int32_t *senders;         // [L*K]   senders of each receiver, ascending
+  float *alpha;             // [L*K]   mixing coefficient of each push, same order
+  unsigned char *flags;     // [L*K]   kFlagActive | kFlagRecv
+};
+
+struct SchedParams {
+  SchedTables t;
+  double *w;                // [L*K] push-sum weights, updated in place
+  uint64_t seed;
+  uint32_t step;
+  uint32_t skip_thr;        // skip iff draw < skip_thr; 0 = straggler mode off
+  int32_t K, L;
+  int32_t layer_begin;      // blockIdx.x + layer_begin = layer
+  int32_t peer_mode;
+};
+
+struct UpdateParams {
+  float *x, *g, *m;                 // section bases (m == nullptr when momentum == 0)
+  const LayerDesc *layers;          // [L]
+  const long long *tile_prefix;     // [L+1] by position; position p holds layer L-1-p
+  SchedTables t;
+  long long tile_begin, tile_end;   // work-list range of this launch
+  int32_t K, L;
+  int32_t C, log2C;                 // float4 columns per tile (power of two)
+  int32_t pos_begin;                // position of tile_begin
+  float neg_lr, mu;
+};
+
+// schedule.cu
+cudaError_t launch_schedule(const SchedParams &p, int n_layers, cudaStream_t s);
+cudaError_t launch_peers_only(uint64_t seed, uint32_t step, uint32_t skip_thr, int K, int L, int peer_mode,
+                              int32_t *peer_dev, unsigned char *active_dev, cudaStream_t s);
+// update.cu
+cudaError_t update_kernel_setup(int smem_bytes, int *ctas_per_sm);
+cudaError_t launch_update(const UpdateParams &p, int grid, int smem_bytes, cudaStream_t s);
+size_t update_smem_bytes(int K, int C);
+
+}  // namespace layup

@@ -1,0 +1,99 @@
+// Schedule stage: straggler mask, peer choice, push-sum
+// weight halving / adding, and the mixing coefficients, for every layer of a launch.
+// O(L*K) integer + fp64 scalar work; one CTA per layer, one thread per replica.
+//
+// PAPER.md:101  "Randomly select a peer: j ~ Random(M-1);  w_i <- w_i/2;  ...
+//                Peer Update: x^{j,l} <- w_j/(w_i+w_j) x^{j,l} + w_i/(w_i+w_j) x^{i,l};
+//                w_j <- w_j + w_i"
+// Colliding pushes are folded in ascending sender index (R3): for receiver j,
+// alpha_k = wh_i / (W + wh_i), W <- W + wh_i, starting from W = wh_j.
+#include "layup_internal.cuh"
+#include "philox.cuh"
+
+namespace layup {
+
+__global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams p) {
+  extern __shared__ __align__(8) unsigned char sm[];
+  const int K = p.K;
+  double *s_wh = reinterpret_cast<double *>(sm);                 // [K]
+  int *s_peer = reinterpret_cast<int *>(s_wh + K);               // [K]
+  int *s_cnt = s_peer + K;                                       // [K]
+  int *s_off = s_cnt + K;                                        // [K+1]
+
+  const int layer = p.layer_begin + blockIdx.x;
+  const int i = threadIdx.x;
+  const size_t row = (size_t)layer * K;
+
+  bool act = false;
+  if (i < K) {
+    act = draw_active(p.seed, p.step, i, p.skip_thr);
+    int peer = -1;
+    double wh = p.w[row + i];
+    if (act && K >= 2) {
+      peer = draw_peer(p.seed, p.step, p.peer_mode == 0 ? (uint32_t)layer : kNoLayer, i, K);
+      wh = wh * 0.5;                                             // w_i <- w_i / 2 (exact)
+    }
+    s_peer[i] = peer;
+    s_wh[i] = wh;
+    p.t.peer[row + i] = peer;
+  }
+  __syncthreads();
+
+  int cnt = 0;
+  if (i < K) {
+    for (int s = 0; s < K; ++s) cnt += (s_peer[s] == i);
+    s_cnt[i] = cnt;
+  }
+  __syncthreads();
+  if (i == 0) {
+    int run = 0;
+    for (int j = 0; j < K; ++j) { s_off[j] = run; run += s_cnt[j]; }
+    s_off[K] = run;
+  }
+  __syncthreads();
+
+  if (i < K) {
+    double W = s_wh[i];
+    int k = s_off[i];
+    for (int s = 0; s < K; ++s) {
+      if (s_peer[s] != i) continue;
+      const double ws = s_wh[s];
+      p.t.senders[row + k] = s;
+      p.t.alpha[row + k] = (float)(ws / (W + ws));               // one rounding to fp32
+      W = W + ws;                                                // w_j <- w_j + w_i
+      ++k;
+    }
+    p.w[row + i] = W;
+    p.t.flags[row + i] = (unsigned char)((act ? kFlagActive : 0) | (cnt > 0 ? kFlagRecv : 0));
+    p.t.recv_off[(size_t)layer * (K + 1) + i] = s_off[i];
+    if (i == 0) p.t.recv_off[(size_t)layer * (K + 1) + K] = s_off[K];
+  }
+}
+
+// Introspection: peers and mask of an arbitrary round, no state touched.
+__global__ void layup_peers_only_kernel(uint64_t seed, uint32_t step, uint32_t skip_thr, int K, int L,
+                                        int peer_mode, int32_t *peer, unsigned char *active) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= L * K) return;
+  const int layer = idx / K, i = idx - layer * K;
+  const bool act = draw_active(seed, step, i, skip_thr);
+  peer[idx] = (act && K >= 2) ? draw_peer(seed, step, peer_mode == 0 ? (uint32_t)layer : kNoLayer, i, K) : -1;
+  if (layer == 0) active[i] = act ? 1 : 0;
+}
+
+cudaError_t launch_schedule(const SchedParams &p, int n_layers, cudaStream_t s) {
+  const int threads = ((p.K + 31) / 32) * 32;
+  const size_t smem = sizeof(double) * p.K + sizeof(int) * (3 * (size_t)p.K + 1);
+  layup_schedule_kernel<<<n_layers, threads, smem, s>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_peers_only(uint64_t seed, uint32_t step, uint32_t skip_thr, int K, int L, int peer_mode,
+                              int32_t *peer_dev, unsigned char *active_dev, cudaStream_t s) {
+  const int n = K * L;
+  layup_peers_only_kernel<<<(n + 255) / 256, 256, 0, s>>>(seed, step, skip_thr, K, L, peer_mode, peer_dev,
+                                                          active_dev);
+  return cudaGetLastError();
+}
+
+}  // namespace layup

@@ -1,0 +1,96 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/layup.h
+declares, its pure host functions agree with the oracle, and without a GPU it fails
+loudly instead of falling back (no compute calls here)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2410_05985_b200 as pkg
+from paper_2410_05985_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2410_05985_b200.build import build
+    build()
+    return pkg.load_library()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    text = open(os.path.join(ROOT, "include", "layup.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    declared = set(re.findall(r"\b(layup_[a-z_]+)\s*\(", text))
+    assert declared and declared == set(binding.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_header_and_binding_structs_agree(lib):
+    # the ctypes struct mirrors layup_config field by field
+    text = open(os.path.join(ROOT, "include", "layup.h")).read()
+    body = re.search(r"typedef struct \{(.*?)\} layup_config;", text, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = re.findall(r"(\w+)\s*;", body)
+    assert names == [f[0] for f in binding._Config._fields_]
+
+
+def test_arena_bytes_layout():
+    # slices padded to 32 floats, X|G(|M) sections
+    assert pkg.layup_arena_bytes(4, [1, 31, 32, 33], 0.0) == 4 * (32 + 32 + 32 + 64) * 4 * 2
+    assert pkg.layup_arena_bytes(4, [1, 31, 32, 33], 0.9) == 4 * (32 + 32 + 32 + 64) * 4 * 3
+    with pytest.raises(pkg.LayUpError) as e:
+        pkg.layup_arena_bytes(0, [10])
+    assert e.value.code == pkg.LAYUP_EINVAL
+    with pytest.raises(pkg.LayUpError):
+        pkg.layup_arena_bytes(4, [10, 0])
+    with pytest.raises(pkg.LayUpError):
+        pkg.layup_arena_bytes(2000, [10])
+
+
+def test_host_peer_function_matches_oracle():
+    rng = np.random.default_rng(0)
+    for _ in range(3000):
+        K = int(rng.integers(2, 65))
+        seed = int(rng.integers(0, 2**63))
+        step = int(rng.integers(0, 2**32))
+        layer = int(rng.integers(0, 200))
+        rep = int(rng.integers(0, K))
+        assert pkg.layup_peer(seed, step, layer, rep, K) == oracle.peer(seed, step, layer, rep, K, 0)
+        assert pkg.layup_peer(seed, step, -1, rep, K) == oracle.peer(seed, step, layer, rep, K, 1)
+    with pytest.raises(pkg.LayUpError):
+        pkg.layup_peer(0, 0, 0, 0, 1)
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
+def test_no_gpu_means_loud_failure_not_fallback(lib):
+    with pytest.raises(pkg.LayUpError) as e:
+        pkg.LayUp(4, [100], 0.01)
+    assert e.value.code == pkg.LAYUP_ECUDA
+    # and straight through the C-ABI: init must report a CUDA error, never succeed
+    arr = (ctypes.c_int64 * 1)(100)
+    cfg = binding._Config(4, 1, arr, 0.01, 0.0, 0, 0, 0.0, 0)
+    ctx = ctypes.c_void_p()
+    rc = lib.layup_init(ctypes.byref(cfg), ctypes.c_void_p(128), 1 << 20, ctypes.byref(ctx))
+    assert rc == pkg.LAYUP_ECUDA and not ctx.value
+    assert b"cuda" in lib.layup_last_error(None).lower()
+
+
+def test_product_does_not_import_oracle():
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2410_05985_b200")):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", src, flags=re.M), f
+                assert "layup_oracle" not in src and "curand" not in src.lower().replace("does not include curand", ""), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(import|from)\s+paper_2410_05985_b200\b", src, flags=re.M), f
+            assert "#include \"../paper" not in src
