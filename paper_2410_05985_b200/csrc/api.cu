@@ -27,6 +27,8 @@ struct layup_ctx {
   long long section = 0;                  // floats per section
   float *arena = nullptr;
   int C = 0, log2C = 0, smem = 0, ctas_per_sm = 1, n_sm = 1;
+  int variant = 0, threads = 256, launch_shape = -1;   // launch_shape: -1 auto, 0 grouped, 1 persistent
+  int engine = 1;                                      // 1: TMA-staged kernel, 0: LDG kernel
   // device tables
   LayerDesc *d_layers = nullptr;
   long long *d_tile_prefix = nullptr;
@@ -168,7 +170,22 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     fail(nullptr, LAYUP_EINVAL, "K=%d needs %d B of shared memory per CTA", K, ctx->smem);
     return bail(LAYUP_EINVAL);
   }
-  CU_TRY_INIT(update_kernel_setup(ctx->smem, &ctx->ctas_per_sm));
+  ctx->engine = env_int("LAYUP_ENGINE", 1);
+  ctx->variant = env_int("LAYUP_VARIANT", 0);
+  ctx->launch_shape = env_int("LAYUP_PERSISTENT", -1);
+  if (ctx->engine == 1) {
+    // TMA-staged kernel stages x, g (, m) of the whole tile: fall back to the LDG kernel if it does not fit
+    const size_t need_smem = tma_smem_bytes(K, C, cfg->momentum != 0.f);
+    if (need_smem > prop.sharedMemPerBlockOptin) ctx->engine = 0;
+    else ctx->smem = (int)need_smem;
+  }
+  if (ctx->engine == 1) {
+    if (ctx->variant < 0 || ctx->variant >= tma_num_variants()) ctx->variant = 0;
+    CU_TRY_INIT(tma_kernel_setup(ctx->variant, ctx->smem, cfg->momentum != 0.f, &ctx->threads, &ctx->ctas_per_sm));
+  } else {
+    if (ctx->variant < 0 || ctx->variant >= update_num_variants()) ctx->variant = 0;
+    CU_TRY_INIT(update_kernel_setup(ctx->variant, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
+  }
   if (ctx->ctas_per_sm < 1) ctx->ctas_per_sm = 1;
   const int cap = env_int("LAYUP_CTAS_PER_SM", 0);
   if (cap > 0 && cap < ctx->ctas_per_sm) ctx->ctas_per_sm = cap;
@@ -245,10 +262,10 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   up.m = ctx->mu != 0.f ? ctx->arena + 2 * ctx->section : nullptr;
   up.layers = ctx->d_layers; up.tile_prefix = ctx->d_tile_prefix; up.t = ctx->t;
   up.tile_begin = ctx->tile_prefix[pos_begin]; up.tile_end = ctx->tile_prefix[pos_end];
-  up.K = ctx->K; up.L = L; up.C = ctx->C; up.log2C = ctx->log2C; up.pos_begin = pos_begin;
+  up.K = ctx->K; up.L = L; up.C = ctx->C; up.log2C = ctx->log2C; up.pos_begin = pos_begin; up.pos_end = pos_end;
   up.neg_lr = -ctx->lr; up.mu = ctx->mu;
   const long long tiles = up.tile_end - up.tile_begin;
-  const int grid = (int)std::min<long long>(tiles, (long long)ctx->n_sm * ctx->ctas_per_sm);
+  const long long resident = (long long)ctx->n_sm * ctx->ctas_per_sm;
 
   std::pair<cudaEvent_t, cudaEvent_t> ev{nullptr, nullptr};
   if (ctx->profiling) {
@@ -256,12 +273,38 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
     else { CU_TRY(ctx, cudaEventCreate(&ev.first)); CU_TRY(ctx, cudaEventCreate(&ev.second)); }
     CU_TRY(ctx, cudaEventRecord(ev.first, s));
   }
-  CU_TRY(ctx, launch_update(up, grid, ctx->smem, s));
+  int n_launch = 0;
+  if (ctx->engine == 1) {
+    // grouped launch(es): one CTA per work item; the work-list table travels in the kernel parameters
+    for (int q0 = pos_begin; q0 < pos_end;) {
+      PosTable tab;
+      int n = 0;
+      const long long t0 = ctx->tile_prefix[q0];
+      while (q0 + n < pos_end && n < kMaxPos && ctx->tile_prefix[q0 + n + 1] - t0 <= 0x7FFFFFFFll) {
+        tab.prefix[n] = ctx->tile_prefix[q0 + n] - t0;
+        tab.lay[n] = ctx->layers[L - 1 - (q0 + n)];
+        tab.layer[n] = L - 1 - (q0 + n);
+        ++n;
+      }
+      if (n == 0) return fail(ctx, LAYUP_EINVAL, "layer %d has more than 2^31 tiles", L - 1 - q0);
+      tab.prefix[n] = ctx->tile_prefix[q0 + n] - t0;
+      tab.n = n;
+      CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, (int)tab.prefix[n], ctx->smem, s));
+      q0 += n;
+      ++n_launch;
+    }
+  } else {
+    // LDG kernel: grouped (one CTA per work item) unless a persistent grid was asked for
+    const bool persistent = ctx->launch_shape == 1 || tiles > 0x7FFFFFFFll;
+    const int grid = (int)(persistent ? std::min<long long>(tiles, resident) : tiles);
+    CU_TRY(ctx, launch_update(up, ctx->variant, persistent, grid, ctx->smem, s));
+    n_launch = 1;
+  }
   if (ctx->profiling) {
     CU_TRY(ctx, cudaEventRecord(ev.second, s));
     ctx->prof_pending.push_back(ev);
   }
-  ctx->launches += 2;
+  ctx->launches += 1 + n_launch;
   note_stream(ctx, s);
   return LAYUP_OK;
 }

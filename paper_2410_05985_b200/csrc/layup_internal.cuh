@@ -5,7 +5,6 @@
 
 namespace layup {
 
-constexpr int kThreads = 256;          // threads per CTA of the update kernel
 constexpr int kFlagActive = 1;         // replica takes its local step and pushes this round
 constexpr int kFlagRecv = 2;           // replica receives at least one push this round
 
@@ -44,8 +43,19 @@ struct UpdateParams {
   long long tile_begin, tile_end;   // work-list range of this launch
   int32_t K, L;
   int32_t C, log2C;                 // float4 columns per tile (power of two)
-  int32_t pos_begin;                // position of tile_begin
+  int32_t pos_begin, pos_end;       // positions covered by [tile_begin, tile_end)
   float neg_lr, mu;
+};
+
+// Work-list table of one launch, passed by value in the kernel parameters (constant bank):
+// the launch covers positions [0, n) of this table; position q holds layer `layer[q]`
+// (reverse layer order) and the tiles [prefix[q], prefix[q+1]) of the launch.
+constexpr int kMaxPos = 160;
+struct PosTable {
+  long long prefix[kMaxPos + 1];
+  LayerDesc lay[kMaxPos];
+  int32_t layer[kMaxPos];
+  int32_t n;
 };
 
 // schedule.cu
@@ -53,8 +63,16 @@ cudaError_t launch_schedule(const SchedParams &p, int n_layers, cudaStream_t s);
 cudaError_t launch_peers_only(uint64_t seed, uint32_t step, uint32_t skip_thr, int K, int L, int peer_mode,
                               int32_t *peer_dev, unsigned char *active_dev, cudaStream_t s);
 // update.cu
-cudaError_t update_kernel_setup(int smem_bytes, int *ctas_per_sm);
-cudaError_t launch_update(const UpdateParams &p, int grid, int smem_bytes, cudaStream_t s);
+int update_num_variants();
+cudaError_t update_kernel_setup(int variant, int smem_bytes, int *threads, int *ctas_per_sm);
+cudaError_t launch_update(const UpdateParams &p, int variant, bool persistent, int grid, int smem_bytes,
+                          cudaStream_t s);
 size_t update_smem_bytes(int K, int C);
+// update_tma.cu -- TMA-bulk staged variants
+int tma_num_variants();
+size_t tma_smem_bytes(int K, int C, bool mom);
+cudaError_t tma_kernel_setup(int variant, int smem_bytes, bool mom, int *threads, int *ctas_per_sm);
+cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, int grid, int smem_bytes,
+                              cudaStream_t s);
 
 }  // namespace layup

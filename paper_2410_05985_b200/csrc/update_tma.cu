@@ -1,0 +1,198 @@
+// TMA-staged form of the fused local-step + gossip-mix kernel (see update.cu for the rule).
+//
+// Same work item -- (layer, tile of C float4 columns) for ALL K replicas, one CTA per item --
+// but the K x {x, g, m} chunks of the tile are brought into shared memory by 1-D bulk
+// copies (cp.async.bulk, the TMA engine; SASS UBLKCP) completing on one mbarrier, so the
+// whole tile (K*C*16 B * 3) is in flight per CTA without holding registers.  The local step
+// then runs out of shared memory, y overwrites x in place (the "send" is an on-chip read,
+// PAPER.md:101), m' goes straight to HBM, and after one CTA barrier every receiver folds
+// its senders and writes x once.  HBM traffic is unchanged: 12 B / 20 B per parameter update.
+#include "layup_internal.cuh"
+
+namespace layup {
+
+namespace {
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared::cta bulk copy, bytes % 16 == 0, both addresses 16-B aligned
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst_smem)),
+               "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+__device__ __forceinline__ void st4(float *p, const float4 &v) { *reinterpret_cast<float4 *>(p) = v; }
+
+template <bool MOM, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+    layup_update_tma(const __grid_constant__ UpdateParams p, const __grid_constant__ PosTable tab) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int K = p.K, C = p.C, log2C = p.log2C, tid = threadIdx.x;
+  const int n_items = K << log2C;
+  float4 *xs = reinterpret_cast<float4 *>(smem_raw);                       // [K*C]  x, then y in place
+  float4 *gs = xs + n_items;                                                // [K*C]
+  float4 *ms = MOM ? gs + n_items : gs;                                     // [K*C] (momentum only)
+  uint64_t *bar = reinterpret_cast<uint64_t *>((MOM ? ms : gs) + n_items);
+  int *s_recv_off = reinterpret_cast<int *>(bar + 1);                       // [K+1]
+  int *s_senders = s_recv_off + (K + 1);                                    // [K]
+  float *s_alpha = reinterpret_cast<float *>(s_senders + K);                // [K]
+  unsigned char *s_flags = reinterpret_cast<unsigned char *>(s_alpha + K);  // [K]
+
+  if (tid == 0) mbar_init(bar, 1);
+
+  // which layer does this work item belong to: binary search in the parameter table
+  const long long tile = blockIdx.x;
+  int lo = 0, hi = tab.n;
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (tile >= tab.prefix[mid]) lo = mid; else hi = mid;
+  }
+  const int layer = tab.layer[lo];
+  const long long pad = tab.lay[lo].pad;
+  const long long col0 = (tile - tab.prefix[lo]) << log2C;                  // first float4 column
+  const long long cols_left = (pad >> 2) - col0;
+  const int ncols = cols_left < C ? (int)cols_left : C;
+  const long long tile_off = tab.lay[lo].base + (col0 << 2);
+  float *const xb = p.x + tile_off;
+  const float *const gb = p.g + tile_off;
+  float *const mb = MOM ? p.m + tile_off : nullptr;
+
+  // this layer's schedule -> shared memory
+  {
+    const size_t row = (size_t)layer * K;
+    for (int k = tid; k < K; k += THREADS) {
+      s_senders[k] = p.t.senders[row + k];
+      s_alpha[k] = p.t.alpha[row + k];
+      s_flags[k] = p.t.flags[row + k];
+    }
+    for (int k = tid; k <= K; k += THREADS) s_recv_off[k] = p.t.recv_off[(size_t)layer * (K + 1) + k];
+  }
+  __syncthreads();   // schedule + mbarrier init visible
+
+  // producer: warp 0 issues the bulk copies of every replica that is touched this round
+  if (tid < 32) {
+    const uint32_t chunk = (uint32_t)ncols * 16u;
+    uint32_t bytes = 0;
+    for (int i = tid; i < K; i += 32) {
+      const int f = s_flags[i];
+      bytes += f ? chunk * ((f & kFlagActive) ? (MOM ? 3u : 2u) : 1u) : 0u;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xFFFFFFFFu, bytes, o);
+    if (tid == 0) mbar_expect_tx(bar, bytes);
+    __syncwarp();
+    for (int i = tid; i < K; i += 32) {
+      const int f = s_flags[i];
+      if (!f) continue;
+      const long long off = (long long)i * pad;
+      bulk_g2s(xs + (i << log2C), xb + off, chunk, bar);
+      if (f & kFlagActive) {
+        bulk_g2s(gs + (i << log2C), gb + off, chunk, bar);
+        if (MOM) bulk_g2s(ms + (i << log2C), mb + off, chunk, bar);
+      }
+    }
+  }
+  mbar_wait(bar, 0);
+
+  // ---- phase 1: local step out of shared memory; y overwrites x in place, m' -> HBM
+  for (int idx = tid; idx < n_items; idx += THREADS) {
+    const int i = idx >> log2C, c = idx & (C - 1);
+    if (c >= ncols) continue;
+    if (!(s_flags[i] & kFlagActive)) continue;                              // idle replica: y = x already there
+    float4 y = xs[idx];
+    float4 d = gs[idx];
+    if (MOM) {
+      const float4 m = ms[idx];
+      d.x = __fmaf_rn(p.mu, m.x, d.x);
+      d.y = __fmaf_rn(p.mu, m.y, d.y);
+      d.z = __fmaf_rn(p.mu, m.z, d.z);
+      d.w = __fmaf_rn(p.mu, m.w, d.w);
+      st4(mb + (long long)i * pad + (c << 2), d);
+    }
+    y.x = __fmaf_rn(p.neg_lr, d.x, y.x);
+    y.y = __fmaf_rn(p.neg_lr, d.y, y.y);
+    y.z = __fmaf_rn(p.neg_lr, d.z, y.z);
+    y.w = __fmaf_rn(p.neg_lr, d.w, y.w);
+    xs[idx] = y;
+  }
+  __syncthreads();
+
+  // ---- phase 2: each receiver folds its senders in ascending order; x written once
+  for (int idx = tid; idx < n_items; idx += THREADS) {
+    const int i = idx >> log2C, c = idx & (C - 1);
+    if (c >= ncols) continue;
+    if (!s_flags[i]) continue;                                              // idle, no push received: 0 bytes
+    float4 acc = xs[idx];
+    const int k_end = s_recv_off[i + 1];
+    for (int k = s_recv_off[i]; k < k_end; ++k) {
+      const float a = s_alpha[k];
+      const float4 ys = xs[(s_senders[k] << log2C) + c];
+      acc.x = __fmaf_rn(a, __fsub_rn(ys.x, acc.x), acc.x);
+      acc.y = __fmaf_rn(a, __fsub_rn(ys.y, acc.y), acc.y);
+      acc.z = __fmaf_rn(a, __fsub_rn(ys.z, acc.z), acc.z);
+      acc.w = __fmaf_rn(a, __fsub_rn(ys.w, acc.w), acc.w);
+    }
+    st4(xb + (long long)i * pad + (c << 2), acc);
+  }
+}
+
+using TmaFn = void (*)(const UpdateParams, const PosTable);
+struct TmaVariant {
+  int threads, minb;
+  TmaFn fn[2];
+};
+#define LAYUP_TMA_VARIANT(T, MB) TmaVariant{T, MB, {layup_update_tma<false, T, MB>, layup_update_tma<true, T, MB>}}
+const TmaVariant kTma[] = {
+    LAYUP_TMA_VARIANT(256, 4), LAYUP_TMA_VARIANT(128, 8), LAYUP_TMA_VARIANT(512, 2), LAYUP_TMA_VARIANT(256, 2),
+    LAYUP_TMA_VARIANT(128, 4), LAYUP_TMA_VARIANT(256, 8), LAYUP_TMA_VARIANT(64, 16),
+};
+constexpr int kNumTma = sizeof(kTma) / sizeof(kTma[0]);
+
+}  // namespace
+
+int tma_num_variants() { return kNumTma; }
+
+size_t tma_smem_bytes(int K, int C, bool mom) {
+  return (size_t)K * C * sizeof(float4) * (mom ? 3 : 2) + 8 + sizeof(int) * (2 * (size_t)K + 1) + sizeof(float) * K + (size_t)K;
+}
+
+cudaError_t tma_kernel_setup(int variant, int smem_bytes, bool mom, int *threads, int *ctas_per_sm) {
+  if (variant < 0 || variant >= kNumTma) return cudaErrorInvalidValue;
+  const TmaVariant &v = kTma[variant];
+  TmaFn f = v.fn[mom ? 1 : 0];
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
+  int a = 0;
+  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, f, v.threads, smem_bytes)) != cudaSuccess) return e;
+  *threads = v.threads;
+  *ctas_per_sm = a;
+  return cudaSuccess;
+}
+
+cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, int grid, int smem_bytes,
+                              cudaStream_t s) {
+  const TmaVariant &v = kTma[variant];
+  v.fn[p.m != nullptr ? 1 : 0]<<<grid, v.threads, smem_bytes, s>>>(p, tab);
+  return cudaGetLastError();
+}
+
+}  // namespace layup
