@@ -130,10 +130,14 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   ctx->arena = (float *)arena_dev;
   ctx->section = section_floats(cfg);
 
-  // tile shape: C float4 columns per replica, K*C items per tile
-  const int items_target = std::max(256, env_int("LAYUP_TILE_ITEMS", 1024));
+  // tile shape: C float4 columns per replica (power of two, >= 8), K*C items per tile.
+  // ~1024 items (48 KB staged with momentum, 4 CTAs/SM) measured best on B200; chunks are
+  // kept >= 512 B per replica when the staging still fits comfortably (large K, no momentum).
+  const int items_env = env_int("LAYUP_TILE_ITEMS", 0);
+  const int items_target = std::max(256, items_env > 0 ? items_env : 1024);
   int C = 8;
   while ((long long)cfg->K * C * 2 <= items_target && C < 4096) C *= 2;
+  if (items_env <= 0 && cfg->momentum == 0.f && C < 32 && cfg->K <= 64) C = 32;
   ctx->C = C;
   ctx->log2C = 0;
   while ((1 << ctx->log2C) < C) ++ctx->log2C;
@@ -263,7 +267,7 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   up.layers = ctx->d_layers; up.tile_prefix = ctx->d_tile_prefix; up.t = ctx->t;
   up.tile_begin = ctx->tile_prefix[pos_begin]; up.tile_end = ctx->tile_prefix[pos_end];
   up.K = ctx->K; up.L = L; up.C = ctx->C; up.log2C = ctx->log2C; up.pos_begin = pos_begin; up.pos_end = pos_end;
-  up.neg_lr = -ctx->lr; up.mu = ctx->mu;
+  up.neg_lr = -ctx->lr; up.mu = ctx->mu; up.all_active = ctx->skip_thr == 0u ? 1 : 0;
   const long long tiles = up.tile_end - up.tile_begin;
   const long long resident = (long long)ctx->n_sm * ctx->ctas_per_sm;
 

@@ -45,6 +45,7 @@ struct UpdateParams {
   int32_t C, log2C;                 // float4 columns per tile (power of two)
   int32_t pos_begin, pos_end;       // positions covered by [tile_begin, tile_end)
   float neg_lr, mu;
+  int32_t all_active;               // skip_prob == 0: every replica is active in every round
 };
 
 // Work-list table of one launch, passed by value in the kernel parameters (constant bank):

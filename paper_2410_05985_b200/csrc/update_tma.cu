@@ -56,8 +56,6 @@ __global__ void __launch_bounds__(THREADS, MINB)
   float *s_alpha = reinterpret_cast<float *>(s_senders + K);                // [K]
   unsigned char *s_flags = reinterpret_cast<unsigned char *>(s_alpha + K);  // [K]
 
-  if (tid == 0) mbar_init(bar, 1);
-
   // which layer does this work item belong to: binary search in the parameter table
   const long long tile = blockIdx.x;
   int lo = 0, hi = tab.n;
@@ -74,8 +72,36 @@ __global__ void __launch_bounds__(THREADS, MINB)
   float *const xb = p.x + tile_off;
   const float *const gb = p.g + tile_off;
   float *const mb = MOM ? p.m + tile_off : nullptr;
+  const uint32_t chunk = (uint32_t)ncols * 16u;
+  constexpr int NARR = MOM ? 3 : 2;
 
-  // this layer's schedule -> shared memory
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    // no straggler this round: every replica is active, the byte count is known up front
+    if (p.all_active) mbar_expect_tx(bar, (uint32_t)K * NARR * chunk);
+  }
+  __syncthreads();   // mbarrier visible
+
+  // Bulk copies are issued one lane at a time within a warp, so spread them over all warps:
+  // copy slot c = (replica, array) goes to warp c % NW, lane c / NW.
+  constexpr int NW = THREADS / 32;
+  const int slot0 = (tid & 31) * NW + (tid >> 5);
+  auto issue_copies = [&](bool use_flags) {
+    for (int c = slot0; c < K * NARR; c += THREADS) {
+      const int i = c / NARR, a = c - i * NARR;
+      if (use_flags) {
+        const int f = s_flags[i];
+        if (!f || (a > 0 && !(f & kFlagActive))) continue;
+      }
+      const long long off = (long long)i * pad;
+      if (a == 0) bulk_g2s(xs + (i << log2C), xb + off, chunk, bar);
+      else if (a == 1) bulk_g2s(gs + (i << log2C), gb + off, chunk, bar);
+      else bulk_g2s(ms + (i << log2C), mb + off, chunk, bar);
+    }
+  };
+  if (p.all_active) issue_copies(false);
+
+  // this layer's schedule -> shared memory (overlaps the bulk copies when all replicas are active)
   {
     const size_t row = (size_t)layer * K;
     for (int k = tid; k < K; k += THREADS) {
@@ -85,30 +111,22 @@ __global__ void __launch_bounds__(THREADS, MINB)
     }
     for (int k = tid; k <= K; k += THREADS) s_recv_off[k] = p.t.recv_off[(size_t)layer * (K + 1) + k];
   }
-  __syncthreads();   // schedule + mbarrier init visible
+  __syncthreads();   // schedule visible
 
-  // producer: warp 0 issues the bulk copies of every replica that is touched this round
-  if (tid < 32) {
-    const uint32_t chunk = (uint32_t)ncols * 16u;
-    uint32_t bytes = 0;
-    for (int i = tid; i < K; i += 32) {
-      const int f = s_flags[i];
-      bytes += f ? chunk * ((f & kFlagActive) ? (MOM ? 3u : 2u) : 1u) : 0u;
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xFFFFFFFFu, bytes, o);
-    if (tid == 0) mbar_expect_tx(bar, bytes);
-    __syncwarp();
-    for (int i = tid; i < K; i += 32) {
-      const int f = s_flags[i];
-      if (!f) continue;
-      const long long off = (long long)i * pad;
-      bulk_g2s(xs + (i << log2C), xb + off, chunk, bar);
-      if (f & kFlagActive) {
-        bulk_g2s(gs + (i << log2C), gb + off, chunk, bar);
-        if (MOM) bulk_g2s(ms + (i << log2C), mb + off, chunk, bar);
+  if (!p.all_active) {
+    // straggler round: the flags decide which chunks are touched at all
+    if (tid < 32) {
+      uint32_t bytes = 0;
+      for (int i = tid; i < K; i += 32) {
+        const int f = s_flags[i];
+        bytes += f ? chunk * ((f & kFlagActive) ? (uint32_t)NARR : 1u) : 0u;
       }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xFFFFFFFFu, bytes, o);
+      if (tid == 0) mbar_expect_tx(bar, bytes);
     }
+    __syncthreads();
+    issue_copies(true);
   }
   mbar_wait(bar, 0);
 
