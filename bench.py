@@ -73,13 +73,15 @@ def measured_peak():
 
 
 def committed_traffic(name):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture
+    (profiles/traffic.csv, see profiles/traffic.md); None if this workload was not captured."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(p):
-        try:
-            return json.load(open(p)).get(name)
-        except Exception:
-            pass
+        import csv
+        with open(p) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == name:
+                    return float(row["dram_bytes_per_launch"])
     return None
 
 
@@ -153,7 +155,7 @@ class ClockSampler:
         self.rows, self.proc = [], None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -202,6 +204,18 @@ def algorithmic_bytes(w, lu, steps_range):
                 b += 8 * numel[recv].sum()
         bts.append(b); ups.append(u)
     return bts, ups
+
+
+def reduce_over_ranks(dist, ms, updates, nbytes, device):
+    """Replicas-only aggregation: time = MAX over ranks, work = SUM over ranks.
+    dist is torch.distributed (any backend) or None for a single process."""
+    if dist is None:
+        return float(ms), float(updates), float(nbytes)
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    tot = torch.tensor([updates, nbytes], device=device, dtype=torch.float64)
+    dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(tot[0].item()), float(tot[1].item())
 
 
 def run_ours(args, w, rank, world, local_rank):
@@ -263,15 +277,7 @@ def run_ours(args, w, rank, world, local_rank):
     clocks = sampler.summary(t0, t1) if sampler else None
     bts, ups = algorithmic_bytes(w, lu, range(first, first + args.steps))
 
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-        tot = torch.tensor([sum(ups), sum(bts)], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        job_updates, job_bytes = float(tot[0].item()), float(tot[1].item())
-    else:
-        job_updates, job_bytes = float(sum(ups)), float(sum(bts))
+    ms, job_updates, job_bytes = reduce_over_ranks(dist, ms, sum(ups), sum(bts), torch.device("cuda", local_rank))
     value = job_updates / (ms * 1e-3)
     eff_gbs = job_bytes / (ms * 1e-3) / 1e9
 
