@@ -29,6 +29,7 @@ struct layup_ctx {
   int C = 0, log2C = 0, smem = 0, ctas_per_sm = 1, n_sm = 1;
   int variant = 0, threads = 256, launch_shape = -1;   // launch_shape: -1 auto, 0 grouped, 1 persistent
   int engine = 1;                                      // 1: TMA-staged kernel, 0: LDG kernel
+  int hints = 0;                                       // cache-hint bits of UpdateParams::hints
   // device tables
   LayerDesc *d_layers = nullptr;
   long long *d_tile_prefix = nullptr;
@@ -175,6 +176,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     return bail(LAYUP_EINVAL);
   }
   ctx->engine = env_int("LAYUP_ENGINE", 1);
+  ctx->hints = env_int("LAYUP_HINTS", 0);
   ctx->variant = env_int("LAYUP_VARIANT", 0);
   ctx->launch_shape = env_int("LAYUP_PERSISTENT", -1);
   if (ctx->engine == 1) {
@@ -268,6 +270,7 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   up.tile_begin = ctx->tile_prefix[pos_begin]; up.tile_end = ctx->tile_prefix[pos_end];
   up.K = ctx->K; up.L = L; up.C = ctx->C; up.log2C = ctx->log2C; up.pos_begin = pos_begin; up.pos_end = pos_end;
   up.neg_lr = -ctx->lr; up.mu = ctx->mu; up.all_active = ctx->skip_thr == 0u ? 1 : 0;
+  up.hints = ctx->hints;
   const long long tiles = up.tile_end - up.tile_begin;
   const long long resident = (long long)ctx->n_sm * ctx->ctas_per_sm;
 

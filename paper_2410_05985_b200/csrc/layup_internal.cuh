@@ -46,6 +46,7 @@ struct UpdateParams {
   int32_t pos_begin, pos_end;       // positions covered by [tile_begin, tile_end)
   float neg_lr, mu;
   int32_t all_active;               // skip_prob == 0: every replica is active in every round
+  int32_t hints;                    // bit 0: L2 evict-first on bulk loads; bit 1: streaming stores
 };
 
 // Work-list table of one launch, passed by value in the kernel parameters (constant bank):

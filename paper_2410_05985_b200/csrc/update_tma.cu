@@ -39,7 +39,23 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
                : "memory");
 }
 
+// same copy with an L2 evict-first policy: every byte of the arena is touched once per round
+__device__ __forceinline__ void bulk_g2s_ef(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar,
+                                            uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(dst_smem)),
+      "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+      : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+
 __device__ __forceinline__ void st4(float *p, const float4 &v) { *reinterpret_cast<float4 *>(p) = v; }
+__device__ __forceinline__ void st4_cs(float *p, const float4 &v) { __stcs(reinterpret_cast<float4 *>(p), v); }
 
 template <bool MOM, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
@@ -94,9 +110,10 @@ __global__ void __launch_bounds__(THREADS, MINB)
         if (!f || (a > 0 && !(f & kFlagActive))) continue;
       }
       const long long off = (long long)i * pad;
-      if (a == 0) bulk_g2s(xs + (i << log2C), xb + off, chunk, bar);
-      else if (a == 1) bulk_g2s(gs + (i << log2C), gb + off, chunk, bar);
-      else bulk_g2s(ms + (i << log2C), mb + off, chunk, bar);
+      void *dst = a == 0 ? xs + (i << log2C) : a == 1 ? gs + (i << log2C) : ms + (i << log2C);
+      const float *src = a == 0 ? xb + off : a == 1 ? gb + off : mb + off;
+      if (p.hints & 1) bulk_g2s_ef(dst, src, chunk, bar, policy_evict_first());
+      else bulk_g2s(dst, src, chunk, bar);
     }
   };
   if (p.all_active) issue_copies(false);
@@ -143,7 +160,7 @@ __global__ void __launch_bounds__(THREADS, MINB)
       d.y = __fmaf_rn(p.mu, m.y, d.y);
       d.z = __fmaf_rn(p.mu, m.z, d.z);
       d.w = __fmaf_rn(p.mu, m.w, d.w);
-      st4(mb + (long long)i * pad + (c << 2), d);
+      if (p.hints & 2) st4_cs(mb + (long long)i * pad + (c << 2), d); else st4(mb + (long long)i * pad + (c << 2), d);
     }
     y.x = __fmaf_rn(p.neg_lr, d.x, y.x);
     y.y = __fmaf_rn(p.neg_lr, d.y, y.y);
@@ -168,7 +185,7 @@ __global__ void __launch_bounds__(THREADS, MINB)
       acc.z = __fmaf_rn(a, __fsub_rn(ys.z, acc.z), acc.z);
       acc.w = __fmaf_rn(a, __fsub_rn(ys.w, acc.w), acc.w);
     }
-    st4(xb + (long long)i * pad + (c << 2), acc);
+    if (p.hints & 2) st4_cs(xb + (long long)i * pad + (c << 2), acc); else st4(xb + (long long)i * pad + (c << 2), acc);
   }
 }
 
