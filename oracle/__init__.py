@@ -39,13 +39,17 @@ def lib():
         _lib.oracle_active.restype = c.c_int32
         _lib.oracle_peer.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_int32, c.c_int32]
         _lib.oracle_peer.restype = c.c_int32
+        _lib.oracle_active_ex.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_float, c.c_int32, c.c_int32]
+        _lib.oracle_active_ex.restype = c.c_int32
         _lib.oracle_schedule.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_int32, c.c_float,
-                                         c.c_void_p, c.c_void_p]
+                                         c.c_int32, c.c_int32, c.c_void_p, c.c_void_p]
+        _lib.oracle_disagreement.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p]
+        _lib.oracle_disagreement.restype = None
         _lib.oracle_schedule.restype = None
         for name, ft in (("oracle_layer_update", c.c_float), ("oracle_layer_update_f64", c.c_double)):
             f = getattr(_lib, name)
             f.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
-                          ft, ft, c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_float,
+                          ft, ft, c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_int32,
                           c.c_void_p, c.c_void_p]
             f.restype = c.c_int
     return _lib
@@ -63,24 +67,35 @@ def philox4x32_10(ctr, key):
     return out
 
 
-def active(seed, step, replica, skip_prob):
-    return int(lib().oracle_active(seed, step, replica, skip_prob))
+def active(seed, step, replica, skip_prob, delay_replica=0, delay_rounds=0):
+    return int(lib().oracle_active_ex(seed, step, replica, skip_prob, delay_replica, delay_rounds))
 
 
 def peer(seed, step, layer, replica, K, peer_mode=0):
     return int(lib().oracle_peer(seed, step, layer, replica, K, peer_mode))
 
 
-def schedule(seed, step, L, K, peer_mode=0, skip_prob=0.0):
+def schedule(seed, step, L, K, peer_mode=0, skip_prob=0.0, delay_replica=0, delay_rounds=0):
     """-> (peer[L,K] int32 with -1 for inactive replicas, active[K] uint8)."""
     p = np.empty((L, K), dtype=np.int32)
     a = np.empty(K, dtype=np.uint8)
-    lib().oracle_schedule(seed, step, L, K, peer_mode, skip_prob, _ptr(p), _ptr(a))
+    lib().oracle_schedule(seed, step, L, K, peer_mode, skip_prob, delay_replica, delay_rounds, _ptr(p), _ptr(a))
     return p, a
 
 
+def disagreement(x, w=None):
+    """dist[i] = ||x_i - xbar||^2 over one layer; x: [K, n] fp32; w: [K] fp64 weights or None (plain mean)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    K, n = x.shape
+    if w is not None:
+        w = np.ascontiguousarray(w, dtype=np.float64)
+    out = np.empty(K, dtype=np.float64)
+    lib().oracle_disagreement(K, n, _ptr(x), _ptr(w), _ptr(out))
+    return out
+
+
 def layer_update(x, g, m, w, lr, mu, seed, step, layer, peer_mode=0, skip_prob=0.0,
-                 peer_in=None, active_in=None):
+                 peer_in=None, active_in=None, delay_replica=0, delay_rounds=0):
     """One (step, layer) in place.  x, g, m: [K, n] (fp32, or x/m fp64 for the shadow); w: [K] fp64."""
     K, n = x.shape
     f64 = x.dtype == np.float64
@@ -94,7 +109,7 @@ def layer_update(x, g, m, w, lr, mu, seed, step, layer, peer_mode=0, skip_prob=0
         active_in = np.ascontiguousarray(active_in, dtype=np.uint8)
     f = lib().oracle_layer_update_f64 if f64 else lib().oracle_layer_update
     rc = f(K, n, _ptr(x), _ptr(g), _ptr(m) if mu != 0.0 else None, _ptr(w), lr, mu, seed, step, layer,
-           peer_mode, skip_prob, _ptr(peer_in), _ptr(active_in))
+           peer_mode, skip_prob, delay_replica, delay_rounds, _ptr(peer_in), _ptr(active_in))
     if rc != 0:
         raise MemoryError("oracle_layer_update failed")
 
@@ -103,11 +118,13 @@ class Oracle:
     """State of K replicas of L layers; round(step, grads) walks the layers L-1 .. 0
     (output layer first)."""
 
-    def __init__(self, numel, K, lr, momentum=0.0, seed=0, peer_mode=0, skip_prob=0.0, f64=False):
+    def __init__(self, numel, K, lr, momentum=0.0, seed=0, peer_mode=0, skip_prob=0.0, f64=False,
+                 delay_replica=0, delay_rounds=0):
         self.numel = [int(n) for n in numel]
         self.L, self.K = len(self.numel), int(K)
         self.lr, self.mu = lr, momentum
         self.seed, self.peer_mode, self.skip_prob = int(seed), int(peer_mode), float(skip_prob)
+        self.delay_replica, self.delay_rounds = int(delay_replica), int(delay_rounds)
         self.dt = np.float64 if f64 else np.float32
         self.x = [np.zeros((self.K, n), dtype=self.dt) for n in self.numel]
         self.m = [np.zeros((self.K, n), dtype=self.dt) for n in self.numel] if momentum != 0.0 else None
@@ -118,7 +135,13 @@ class Oracle:
         mu = float(np.float32(self.mu)) if self.dt == np.float64 else self.mu
         layer_update(self.x[layer], np.ascontiguousarray(g, dtype=np.float32),
                      self.m[layer] if self.m is not None else None, self.w[layer],
-                     lr, mu, self.seed, step, layer, self.peer_mode, self.skip_prob)
+                     lr, mu, self.seed, step, layer, self.peer_mode, self.skip_prob,
+                     delay_replica=self.delay_replica, delay_rounds=self.delay_rounds)
+
+    def disagreement(self, weighted=False):
+        """[L, K] squared distances to the (weighted) consensus, per layer."""
+        return np.stack([disagreement(np.asarray(self.x[l], dtype=np.float32), self.w[l] if weighted else None)
+                         for l in range(self.L)])
 
     def round(self, step, grads):
         for layer in reversed(range(self.L)):

@@ -88,6 +88,19 @@ int32_t oracle_active(uint64_t seed, int64_t step, int32_t replica, float skip_p
   return r < thr ? 0 : 1;
 }
 
+/* Delay-mode straggler (reading R19; "one device (straggler) is caused to operate
+ * slower ... by forcing it to idle. The idle time is chosen to be a multiple of the time required
+ * ... to perform one forward and one backward pass ... delays are expressed in terms of the number
+ * of iterations the straggler lags behind"): replica delay_replica completes one iteration every
+ * delay_rounds+1 rounds -- it is active only in rounds t with (t+1) % (delay_rounds+1) == 0 -- and
+ * idles (still receiving) in between.  delay_rounds == 0: off.  Combined with the
+ * random mask by AND.                                                                        */
+int32_t oracle_active_ex(uint64_t seed, int64_t step, int32_t replica, float skip_prob,
+                         int32_t delay_replica, int32_t delay_rounds) {
+  if (delay_rounds > 0 && replica == delay_replica && ((step + 1) % ((int64_t)delay_rounds + 1)) != 0) return 0;
+  return oracle_active(seed, step, replica, skip_prob);
+}
+
 /* PAPER.md:101 "j ~ Random(M-1)": uniform over the K-1 other workers (R5).
  * uint32 -> [0, K-2] by multiply-high (R6), then skip over self.
  * peer_mode 0: a fresh peer per (step, layer, replica) (BASELINE.json north_star)
@@ -103,8 +116,10 @@ int32_t oracle_peer(uint64_t seed, int64_t step, int32_t layer, int32_t replica,
 
 /* peer[l*K+i] = chosen peer, or -1 when replica i is inactive (or K == 1). */
 void oracle_schedule(uint64_t seed, int64_t step, int32_t L, int32_t K, int32_t peer_mode,
-                     float skip_prob, int32_t *peer, uint8_t *active) {
-  for (int32_t i = 0; i < K; ++i) active[i] = (uint8_t)oracle_active(seed, step, i, skip_prob);
+                     float skip_prob, int32_t delay_replica, int32_t delay_rounds,
+                     int32_t *peer, uint8_t *active) {
+  for (int32_t i = 0; i < K; ++i)
+    active[i] = (uint8_t)oracle_active_ex(seed, step, i, skip_prob, delay_replica, delay_rounds);
   for (int32_t l = 0; l < L; ++l)
     for (int32_t i = 0; i < K; ++i)
       peer[(size_t)l * K + i] = active[i] ? oracle_peer(seed, step, l, i, K, peer_mode) : -1;
@@ -117,7 +132,7 @@ void oracle_schedule(uint64_t seed, int64_t step, int32_t L, int32_t K, int32_t 
  * Returns 0, or -1 on allocation failure.                                    */
 int oracle_layer_update(int32_t K, int64_t n, float *x, const float *g, float *m, double *w,
                         float lr, float mu, uint64_t seed, int64_t step, int32_t layer,
-                        int32_t peer_mode, float skip_prob,
+                        int32_t peer_mode, float skip_prob, int32_t delay_replica, int32_t delay_rounds,
                         const int32_t *peer_in, const uint8_t *active_in) {
   int32_t *peer = (int32_t *)malloc(sizeof(int32_t) * (size_t)K);
   uint8_t *active = (uint8_t *)malloc((size_t)K);
@@ -131,7 +146,8 @@ int oracle_layer_update(int32_t K, int64_t n, float *x, const float *g, float *m
 
   /* 1. straggler mask; 2. peer choice and weight halving */
   for (int32_t i = 0; i < K; ++i) {
-    active[i] = active_in ? active_in[i] : (uint8_t)oracle_active(seed, step, i, skip_prob);
+    active[i] = active_in ? active_in[i]
+                          : (uint8_t)oracle_active_ex(seed, step, i, skip_prob, delay_replica, delay_rounds);
     if (active[i] && K >= 2) {
       peer[i] = peer_in ? peer_in[i] : oracle_peer(seed, step, layer, i, K, peer_mode);
       wh[i] = w[i] * 0.5;
@@ -192,7 +208,7 @@ int oracle_layer_update(int32_t K, int64_t n, float *x, const float *g, float *m
  * Used for the 100-round error bound and as an independent statement of step 4. */
 int oracle_layer_update_f64(int32_t K, int64_t n, double *x, const float *g, double *m, double *w,
                             double lr, double mu, uint64_t seed, int64_t step, int32_t layer,
-                            int32_t peer_mode, float skip_prob,
+                            int32_t peer_mode, float skip_prob, int32_t delay_replica, int32_t delay_rounds,
                             const int32_t *peer_in, const uint8_t *active_in) {
   int32_t *peer = (int32_t *)malloc(sizeof(int32_t) * (size_t)K);
   uint8_t *active = (uint8_t *)malloc((size_t)K);
@@ -203,7 +219,8 @@ int oracle_layer_update_f64(int32_t K, int64_t n, double *x, const float *g, dou
     return -1;
   }
   for (int32_t i = 0; i < K; ++i) {
-    active[i] = active_in ? active_in[i] : (uint8_t)oracle_active(seed, step, i, skip_prob);
+    active[i] = active_in ? active_in[i]
+                          : (uint8_t)oracle_active_ex(seed, step, i, skip_prob, delay_replica, delay_rounds);
     if (active[i] && K >= 2) {
       peer[i] = peer_in ? peer_in[i] : oracle_peer(seed, step, layer, i, K, peer_mode);
       wh[i] = w[i] * 0.5;
@@ -247,4 +264,21 @@ int oracle_layer_update_f64(int32_t K, int64_t n, double *x, const float *g, dou
   }
   free(peer); free(active); free(wh); free(y);
   return 0;
+}
+
+/* ---- model disagreement (PAPER.md:389-395 Fig. A1; eq. (9)
+ * E||xbar_t - x_t^i||^2 <= eta^2 B^2): per replica, the squared distance to the consensus
+ *     dist[i] = sum_e (x_i[e] - xbar[e])^2 ,  xbar[e] = sum_i c_i x_i[e]
+ * with c_i = 1/K (the paper's plain average, w == NULL) or c_i = w_i (push-sum weighted
+ * consensus, sum_i w_i = 1).  x: [K][n] fp32; everything accumulated in fp64.             */
+void oracle_disagreement(int32_t K, int64_t n, const float *x, const double *w, double *dist) {
+  for (int32_t i = 0; i < K; ++i) dist[i] = 0.0;
+  for (int64_t e = 0; e < n; ++e) {
+    double xbar = 0.0;
+    for (int32_t i = 0; i < K; ++i) xbar += (w ? w[i] : 1.0 / (double)K) * (double)x[(size_t)i * n + e];
+    for (int32_t i = 0; i < K; ++i) {
+      const double d = (double)x[(size_t)i * n + e] - xbar;
+      dist[i] += d * d;
+    }
+  }
 }
