@@ -65,6 +65,10 @@ typedef struct {
                           1: peer per (step, replica), all layers [Alg. 1, PAPER.md:101,453] */
   float    skip_prob;  /* straggler mode: P(replica idles this round); 0 = off            */
   int32_t  device;     /* CUDA ordinal                                                    */
+  int32_t  delay_replica; /* delay-mode straggler: this replica ...           */
+  int32_t  delay_rounds;  /* ... completes one iteration every delay_rounds+1 rounds (active
+                          only when (step+1) % (delay_rounds+1) == 0) and keeps receiving in
+                          between; 0 = off.  ANDed with the skip_prob mask    */
 } layup_config;
 
 /* Bytes of device memory the arena needs for this config (X + G (+ M), padded). Pure. */
@@ -124,6 +128,13 @@ int layup_schedule(layup_ctx *ctx, int64_t step, int32_t *peer /*[L*K]*/, uint8_
 
 /* Current push-sum weights w[l*K+i], after all work issued so far. */
 int layup_weights(layup_ctx *ctx, double *w /*[L*K]*/);
+
+/* Model disagreement (PAPER.md:389-395 Fig. A1; eq. (9)): for every layer l and
+ * replica i, dist[l*K+i] = sum_e (x_i[e] - xbar[e])^2, where xbar = (1/K) sum_i x_i (weighted == 0,
+ * the paper's plain average) or xbar = sum_i w_i x_i with the current push-sum weights
+ * (weighted != 0).  Runs a read-only reduction kernel (fp64 accumulation, 4 B of HBM traffic per
+ * parameter) after all work issued so far; dist is a HOST array.  Synchronous. */
+int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist /*[L*K]*/);
 
 /* Device time of the fused update kernel, measured with CUDA events on the launch
  * stream: enable, run, layup_sync(), read (and reset).  launches = update-kernel

@@ -28,12 +28,13 @@ class LayUpError(RuntimeError):
 class _Config(ctypes.Structure):
     _fields_ = [("K", ctypes.c_int32), ("L", ctypes.c_int32), ("numel", ctypes.POINTER(ctypes.c_int64)),
                 ("lr", ctypes.c_float), ("momentum", ctypes.c_float), ("seed", ctypes.c_uint64),
-                ("peer_mode", ctypes.c_int32), ("skip_prob", ctypes.c_float), ("device", ctypes.c_int32)]
+                ("peer_mode", ctypes.c_int32), ("skip_prob", ctypes.c_float), ("device", ctypes.c_int32),
+                ("delay_replica", ctypes.c_int32), ("delay_rounds", ctypes.c_int32)]
 
 
 EXPORTS = ["layup_arena_bytes", "layup_init", "layup_destroy", "layup_ptr", "layup_set_lr",
            "layup_layer_update", "layup_round", "layup_round_host", "layup_sync", "layup_peer",
-           "layup_schedule", "layup_weights", "layup_profile", "layup_profile_read", "layup_launch_count",
+           "layup_schedule", "layup_weights", "layup_disagreement", "layup_profile", "layup_profile_read", "layup_launch_count",
            "layup_last_error"]
 
 
@@ -60,6 +61,7 @@ def load_library():
         "layup_peer": [c.c_uint64, i64, i32, i32, i32, c.POINTER(i32)],
         "layup_schedule": [vp, i64, vp, vp],
         "layup_weights": [vp, vp],
+        "layup_disagreement": [vp, i32, vp],
         "layup_profile": [vp, i32],
         "layup_profile_read": [vp, c.POINTER(i64), c.POINTER(c.c_double)],
         "layup_launch_count": [vp, c.POINTER(i64)],
@@ -77,10 +79,10 @@ def _check(rc, ctx=None):
         raise LayUpError(rc, (load_library().layup_last_error(ctx) or b"").decode())
 
 
-def _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device):
+def _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device, delay_replica=0, delay_rounds=0):
     arr = (ctypes.c_int64 * len(numel))(*[int(n) for n in numel])
     cfg = _Config(int(K), len(numel), arr, float(lr), float(momentum), int(seed), int(peer_mode),
-                  float(skip_prob), int(device))
+                  float(skip_prob), int(device), int(delay_replica), int(delay_rounds))
     cfg._keep = arr
     return cfg
 
@@ -110,12 +112,13 @@ class LayUp:
     """One ctx = K replicas of L layers in one torch-allocated arena on one GPU."""
 
     def __init__(self, K: int, numel: Sequence[int], lr: float, momentum: float = 0.0, seed: int = 0,
-                 peer_mode: int = 0, skip_prob: float = 0.0, device: int = 0):
+                 peer_mode: int = 0, skip_prob: float = 0.0, device: int = 0,
+                 delay_replica: int = 0, delay_rounds: int = 0):
         self.lib = load_library()
         self.K, self.L, self.numel = int(K), len(numel), [int(n) for n in numel]
         self.momentum = float(momentum)
         self.device = torch.device("cuda", device)
-        self._cfg = _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device)
+        self._cfg = _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device, delay_replica, delay_rounds)
         nbytes = ctypes.c_size_t(0)
         _check(self.lib.layup_arena_bytes(ctypes.byref(self._cfg), ctypes.byref(nbytes)))
         self.arena_bytes = nbytes.value
@@ -175,6 +178,11 @@ class LayUp:
         w = np.empty((self.L, self.K), dtype=np.float64)
         _check(self.lib.layup_weights(self.ctx, w.ctypes.data), self.ctx)
         return w
+
+    def layup_disagreement(self, weighted: bool = False) -> np.ndarray:
+        d = np.empty((self.L, self.K), dtype=np.float64)
+        _check(self.lib.layup_disagreement(self.ctx, 1 if weighted else 0, d.ctypes.data), self.ctx)
+        return d
 
     def layup_profile(self, enable: bool):
         _check(self.lib.layup_profile(self.ctx, 1 if enable else 0), self.ctx)

@@ -30,6 +30,9 @@ struct layup_ctx {
   int variant = 0, threads = 256, launch_shape = -1;   // launch_shape: -1 auto, 0 grouped, 1 persistent
   int engine = 1;                                      // 1: TMA-staged kernel, 0: LDG kernel
   int hints = 0;                                       // cache-hint bits of UpdateParams::hints
+  int32_t delay_replica = 0, delay_rounds = 0;
+  int diag_C = 0, diag_log2C = 0, diag_smem = 0, diag_ctas = 1;
+  double *d_dist = nullptr;
   // device tables
   LayerDesc *d_layers = nullptr;
   long long *d_tile_prefix = nullptr;
@@ -79,6 +82,8 @@ static int check_config(const layup_config *cfg) {
   if (!(cfg->skip_prob >= 0.f && cfg->skip_prob <= 1.f)) return fail(nullptr, LAYUP_EINVAL, "skip_prob outside [0,1]");
   if (cfg->peer_mode != 0 && cfg->peer_mode != 1) return fail(nullptr, LAYUP_EINVAL, "peer_mode must be 0 or 1");
   if (!(cfg->momentum >= 0.f) || !(cfg->lr == cfg->lr)) return fail(nullptr, LAYUP_EINVAL, "lr / momentum invalid");
+  if (cfg->delay_rounds < 0 || (cfg->delay_rounds > 0 && (cfg->delay_replica < 0 || cfg->delay_replica >= cfg->K)))
+    return fail(nullptr, LAYUP_EINVAL, "delay_replica / delay_rounds invalid");
   return LAYUP_OK;
 }
 
@@ -128,6 +133,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     if (th > 4294967295.0) th = 4294967295.0;
     ctx->skip_thr = cfg->skip_prob > 0.f ? (uint32_t)th : 0u;
   }
+  ctx->delay_replica = cfg->delay_replica; ctx->delay_rounds = cfg->delay_rounds;
   ctx->arena = (float *)arena_dev;
   ctx->section = section_floats(cfg);
 
@@ -207,6 +213,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   CU_TRY_INIT(cudaMalloc(&ctx->t.flags, (size_t)L * K));
   CU_TRY_INIT(cudaMalloc(&ctx->d_peer_scratch, sizeof(int32_t) * L * K));
   CU_TRY_INIT(cudaMalloc(&ctx->d_active_scratch, (size_t)K));
+  CU_TRY_INIT(cudaMalloc(&ctx->d_dist, sizeof(double) * L * K));
   CU_TRY_INIT(cudaMemcpy(ctx->d_layers, ctx->layers.data(), sizeof(LayerDesc) * L, cudaMemcpyHostToDevice));
   CU_TRY_INIT(cudaMemcpy(ctx->d_tile_prefix, ctx->tile_prefix.data(), sizeof(long long) * (L + 1), cudaMemcpyHostToDevice));
   std::vector<double> w0((size_t)L * K, 1.0 / (double)K);              // PAPER.md:106  w_i = 1/M
@@ -232,7 +239,7 @@ extern "C" int layup_destroy(layup_ctx *ctx) {
   for (auto &pr : ctx->prof_pool) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
   cudaFree(ctx->d_layers); cudaFree(ctx->d_tile_prefix); cudaFree(ctx->d_w);
   cudaFree(ctx->t.peer); cudaFree(ctx->t.recv_off); cudaFree(ctx->t.senders); cudaFree(ctx->t.alpha);
-  cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_active_scratch);
+  cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_active_scratch); cudaFree(ctx->d_dist);
   delete ctx;
   return LAYUP_OK;
 }
@@ -259,6 +266,7 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   SchedParams sp{};
   sp.t = ctx->t; sp.w = ctx->d_w; sp.seed = ctx->seed; sp.step = (uint32_t)step; sp.skip_thr = ctx->skip_thr;
   sp.K = ctx->K; sp.L = L; sp.peer_mode = ctx->peer_mode;
+  sp.delay_replica = ctx->delay_replica; sp.delay_rounds = ctx->delay_rounds;
   sp.layer_begin = L - pos_end;                       // layers [L-pos_end, L-pos_begin)
   CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
 
@@ -269,7 +277,7 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   up.layers = ctx->d_layers; up.tile_prefix = ctx->d_tile_prefix; up.t = ctx->t;
   up.tile_begin = ctx->tile_prefix[pos_begin]; up.tile_end = ctx->tile_prefix[pos_end];
   up.K = ctx->K; up.L = L; up.C = ctx->C; up.log2C = ctx->log2C; up.pos_begin = pos_begin; up.pos_end = pos_end;
-  up.neg_lr = -ctx->lr; up.mu = ctx->mu; up.all_active = ctx->skip_thr == 0u ? 1 : 0;
+  up.neg_lr = -ctx->lr; up.mu = ctx->mu; up.all_active = (ctx->skip_thr == 0u && ctx->delay_rounds == 0) ? 1 : 0;
   up.hints = ctx->hints;
   const long long tiles = up.tile_end - up.tile_begin;
   const long long resident = (long long)ctx->n_sm * ctx->ctas_per_sm;
@@ -406,7 +414,7 @@ extern "C" int layup_schedule(layup_ctx *ctx, int64_t step, int32_t *peer, uint8
   if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
   CU_TRY(ctx, cudaSetDevice(ctx->device));
   CU_TRY(ctx, launch_peers_only(ctx->seed, (uint32_t)step, ctx->skip_thr, ctx->K, ctx->L, ctx->peer_mode,
-                                ctx->d_peer_scratch, ctx->d_active_scratch, ctx->own_stream));
+                                ctx->delay_replica, ctx->delay_rounds, ctx->d_peer_scratch, ctx->d_active_scratch, ctx->own_stream));
   ctx->launches += 1;
   CU_TRY(ctx, cudaMemcpyAsync(peer, ctx->d_peer_scratch, sizeof(int32_t) * ctx->L * ctx->K, cudaMemcpyDeviceToHost, ctx->own_stream));
   CU_TRY(ctx, cudaMemcpyAsync(active, ctx->d_active_scratch, (size_t)ctx->K, cudaMemcpyDeviceToHost, ctx->own_stream));
@@ -419,6 +427,48 @@ extern "C" int layup_weights(layup_ctx *ctx, double *w) {
   int rc = layup_sync(ctx);
   if (rc) return rc;
   CU_TRY(ctx, cudaMemcpy(w, ctx->d_w, sizeof(double) * ctx->L * ctx->K, cudaMemcpyDeviceToHost));
+  return LAYUP_OK;
+}
+
+extern "C" int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist) {
+  if (!ctx || !dist) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  int rc = layup_sync(ctx);
+  if (rc) return rc;
+  const int K = ctx->K, L = ctx->L;
+  if (ctx->diag_C == 0) {
+    // read-only tile: ~2048 float4 items (32 KB) of x per work item
+    int C = 8;
+    while ((long long)K * C * 2 <= 2048 && C < 1024) C *= 2;
+    ctx->diag_C = C;
+    while ((1 << ctx->diag_log2C) < C) ++ctx->diag_log2C;
+    ctx->diag_smem = (int)diag_smem_bytes(K, C);
+    CU_TRY(ctx, diag_setup(ctx->diag_smem, &ctx->diag_ctas));
+    if (ctx->diag_ctas < 1) return fail(ctx, LAYUP_EINVAL, "K=%d does not fit the diagnostic kernel", K);
+  }
+  cudaStream_t s = ctx->own_stream;
+  CU_TRY(ctx, cudaMemsetAsync(ctx->d_dist, 0, sizeof(double) * L * K, s));
+  const int C = ctx->diag_C;
+  for (int q0 = 0; q0 < L;) {
+    PosTable tab;
+    int n = 0;
+    tab.prefix[0] = 0;
+    while (q0 + n < L && n < kMaxPos) {
+      const LayerDesc &d = ctx->layers[L - 1 - (q0 + n)];
+      tab.lay[n] = d;
+      tab.layer[n] = L - 1 - (q0 + n);
+      tab.prefix[n + 1] = tab.prefix[n] + (d.pad / 4 + C - 1) / C;
+      ++n;
+    }
+    tab.n = n;
+    const long long tiles = tab.prefix[n];
+    const int grid = (int)std::min<long long>(tiles, (long long)ctx->n_sm * ctx->diag_ctas);
+    CU_TRY(ctx, launch_disagreement(ctx->arena, weighted ? ctx->d_w : nullptr, ctx->d_dist, K, C, ctx->diag_log2C,
+                                    tab, grid, ctx->diag_smem, s));
+    ctx->launches += 1;
+    q0 += n;
+  }
+  CU_TRY(ctx, cudaMemcpyAsync(dist, ctx->d_dist, sizeof(double) * L * K, cudaMemcpyDeviceToHost, s));
+  CU_TRY(ctx, cudaStreamSynchronize(s));
   return LAYUP_OK;
 }
 

@@ -33,6 +33,7 @@ struct SchedParams {
   int32_t K, L;
   int32_t layer_begin;      // blockIdx.x + layer_begin = layer
   int32_t peer_mode;
+  int32_t delay_replica, delay_rounds;   // deterministic straggler (0 rounds = off)
 };
 
 struct UpdateParams {
@@ -63,7 +64,13 @@ struct PosTable {
 // schedule.cu
 cudaError_t launch_schedule(const SchedParams &p, int n_layers, cudaStream_t s);
 cudaError_t launch_peers_only(uint64_t seed, uint32_t step, uint32_t skip_thr, int K, int L, int peer_mode,
-                              int32_t *peer_dev, unsigned char *active_dev, cudaStream_t s);
+                              int delay_replica, int delay_rounds, int32_t *peer_dev, unsigned char *active_dev,
+                              cudaStream_t s);
+// diagnose.cu
+size_t diag_smem_bytes(int K, int C);
+cudaError_t diag_setup(int smem_bytes, int *ctas_per_sm);
+cudaError_t launch_disagreement(const float *x, const double *w, double *dist, int K, int C, int log2C,
+                                const PosTable &tab, int grid, int smem_bytes, cudaStream_t s);
 // update.cu
 int update_num_variants();
 cudaError_t update_kernel_setup(int variant, int smem_bytes, int *threads, int *ctas_per_sm);

@@ -52,7 +52,12 @@ LAYUP_HD int32_t draw_peer(uint64_t seed, uint32_t step, uint32_t layer_field, i
 }
 
 // Straggler mask: one draw per (step, replica); skip iff r < thr.
-LAYUP_HD bool draw_active(uint64_t seed, uint32_t step, int32_t replica, uint32_t skip_thr) {
+// Delay mode: replica delay_replica completes one iteration every delay_rounds+1
+// rounds, i.e. is active only when (step+1) % (delay_rounds+1) == 0; ANDed with the random mask.
+LAYUP_HD bool draw_active(uint64_t seed, uint32_t step, int32_t replica, uint32_t skip_thr,
+                          int32_t delay_replica = 0, int32_t delay_rounds = 0) {
+  if (delay_rounds > 0 && replica == delay_replica &&
+      (((uint64_t)step + 1u) % ((uint64_t)delay_rounds + 1u)) != 0u) return false;
   if (skip_thr == 0u) return true;
   const uint32_t r = philox_first_word(step, kNoLayer, (uint32_t)replica, kTagSkip,
                                        (uint32_t)seed, (uint32_t)(seed >> 32));

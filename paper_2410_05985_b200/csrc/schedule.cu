@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
 
   bool act = false;
   if (i < K) {
-    act = draw_active(p.seed, p.step, i, p.skip_thr);
+    act = draw_active(p.seed, p.step, i, p.skip_thr, p.delay_replica, p.delay_rounds);
     int peer = -1;
     double wh = p.w[row + i];
     if (act && K >= 2) {
@@ -72,11 +72,12 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
 
 // Introspection: peers and mask of an arbitrary round, no state touched.
 __global__ void layup_peers_only_kernel(uint64_t seed, uint32_t step, uint32_t skip_thr, int K, int L,
-                                        int peer_mode, int32_t *peer, unsigned char *active) {
+                                        int peer_mode, int delay_replica, int delay_rounds, int32_t *peer,
+                                        unsigned char *active) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= L * K) return;
   const int layer = idx / K, i = idx - layer * K;
-  const bool act = draw_active(seed, step, i, skip_thr);
+  const bool act = draw_active(seed, step, i, skip_thr, delay_replica, delay_rounds);
   peer[idx] = (act && K >= 2) ? draw_peer(seed, step, peer_mode == 0 ? (uint32_t)layer : kNoLayer, i, K) : -1;
   if (layer == 0) active[i] = act ? 1 : 0;
 }
@@ -89,10 +90,11 @@ cudaError_t launch_schedule(const SchedParams &p, int n_layers, cudaStream_t s) 
 }
 
 cudaError_t launch_peers_only(uint64_t seed, uint32_t step, uint32_t skip_thr, int K, int L, int peer_mode,
-                              int32_t *peer_dev, unsigned char *active_dev, cudaStream_t s) {
+                              int delay_replica, int delay_rounds, int32_t *peer_dev, unsigned char *active_dev,
+                              cudaStream_t s) {
   const int n = K * L;
-  layup_peers_only_kernel<<<(n + 255) / 256, 256, 0, s>>>(seed, step, skip_thr, K, L, peer_mode, peer_dev,
-                                                          active_dev);
+  layup_peers_only_kernel<<<(n + 255) / 256, 256, 0, s>>>(seed, step, skip_thr, K, L, peer_mode, delay_replica,
+                                                          delay_rounds, peer_dev, active_dev);
   return cudaGetLastError();
 }
 
