@@ -52,7 +52,28 @@ def lib():
                           ft, ft, c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_int32,
                           c.c_void_p, c.c_void_p]
             f.restype = c.c_int
+        for name in ("oracle_layer_update_ex", "oracle_layer_update_ex_f64"):
+            f = getattr(_lib, name)
+            f.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
+                          c.c_void_p, c.c_void_p, c.POINTER(_Opts), c.c_uint64, c.c_int64, c.c_int32, c.c_int32,
+                          c.c_float, c.c_int32, c.c_int32, c.c_void_p, c.c_void_p]
+            f.restype = c.c_int
     return _lib
+
+
+class _Opts(ctypes.Structure):
+    """oracle_opts of layup_oracle.c (doubles holding fp32-representable values)."""
+    _fields_ = [("optimizer", ctypes.c_int32), ("mix_mode", ctypes.c_int32), ("lr", ctypes.c_double),
+                ("mu", ctypes.c_double), ("wd", ctypes.c_double), ("beta1", ctypes.c_double),
+                ("beta2", ctypes.c_double), ("eps", ctypes.c_double)]
+
+
+OPT_SGD, OPT_ADAMW = 0, 1
+MIX_PUSHSUM, MIX_LOSSY, MIX_SYMMETRIC = 0, 1, 2
+
+
+def _f32(v):
+    return float(np.float32(v))
 
 
 def _ptr(a):
@@ -114,12 +135,44 @@ def layer_update(x, g, m, w, lr, mu, seed, step, layer, peer_mode=0, skip_prob=0
         raise MemoryError("oracle_layer_update failed")
 
 
+def layer_update_ex(x, g, m, v, w, bpow, tcount, lr, mu=0.0, wd=0.0, beta1=0.9, beta2=0.999, eps=1e-8,
+                    optimizer=OPT_SGD, mix_mode=MIX_PUSHSUM, seed=0, step=0, layer=0, peer_mode=0, skip_prob=0.0,
+                    peer_in=None, active_in=None, delay_replica=0, delay_rounds=0):
+    """One (step, layer) of the widened rule (NEXT-3 optimisers, NEXT-4 mixers) in place.
+    x, m, v: [K, n] fp32 (or fp64 for the shadow); g: [K, n] fp32; w: [K] fp64;
+    bpow: [K, 2] fp64 and tcount: [K] int64 (AdamW only, else None)."""
+    K, n = x.shape
+    f64 = x.dtype == np.float64
+    assert x.flags.c_contiguous and g.flags.c_contiguous and w.flags.c_contiguous
+    assert g.dtype == np.float32 and g.shape == x.shape and w.dtype == np.float64 and w.shape == (K,)
+    need_m = optimizer == OPT_ADAMW or mu != 0.0
+    for a, need in ((m, need_m), (v, optimizer == OPT_ADAMW)):
+        if need:
+            assert a is not None and a.dtype == x.dtype and a.shape == x.shape and a.flags.c_contiguous
+    if optimizer == OPT_ADAMW:
+        assert bpow.dtype == np.float64 and bpow.shape == (K, 2) and bpow.flags.c_contiguous
+        assert tcount.dtype == np.int64 and tcount.shape == (K,)
+    if peer_in is not None:
+        peer_in = np.ascontiguousarray(peer_in, dtype=np.int32)
+    if active_in is not None:
+        active_in = np.ascontiguousarray(active_in, dtype=np.uint8)
+    o = _Opts(optimizer, mix_mode, _f32(lr), _f32(mu), _f32(wd), _f32(beta1), _f32(beta2), _f32(eps))
+    f = lib().oracle_layer_update_ex_f64 if f64 else lib().oracle_layer_update_ex
+    rc = f(K, n, _ptr(x), _ptr(g), _ptr(m) if need_m else None, _ptr(v) if optimizer == OPT_ADAMW else None, _ptr(w),
+           _ptr(bpow) if optimizer == OPT_ADAMW else None, _ptr(tcount) if optimizer == OPT_ADAMW else None,
+           ctypes.byref(o), seed, step, layer, peer_mode, skip_prob, delay_replica, delay_rounds,
+           _ptr(peer_in), _ptr(active_in))
+    if rc != 0:
+        raise MemoryError("oracle_layer_update_ex failed")
+
+
 class Oracle:
     """State of K replicas of L layers; round(step, grads) walks the layers L-1 .. 0
     (output layer first)."""
 
     def __init__(self, numel, K, lr, momentum=0.0, seed=0, peer_mode=0, skip_prob=0.0, f64=False,
-                 delay_replica=0, delay_rounds=0):
+                 delay_replica=0, delay_rounds=0, optimizer=OPT_SGD, mix_mode=MIX_PUSHSUM, weight_decay=0.0,
+                 beta1=0.9, beta2=0.999, eps=1e-8):
         self.numel = [int(n) for n in numel]
         self.L, self.K = len(self.numel), int(K)
         self.lr, self.mu = lr, momentum
@@ -127,16 +180,31 @@ class Oracle:
         self.delay_replica, self.delay_rounds = int(delay_replica), int(delay_rounds)
         self.dt = np.float64 if f64 else np.float32
         self.x = [np.zeros((self.K, n), dtype=self.dt) for n in self.numel]
-        self.m = [np.zeros((self.K, n), dtype=self.dt) for n in self.numel] if momentum != 0.0 else None
+        self.optimizer, self.mix_mode, self.wd = int(optimizer), int(mix_mode), float(weight_decay)
+        self.beta1, self.beta2, self.eps = float(beta1), float(beta2), float(eps)
+        adam = self.optimizer == OPT_ADAMW
+        self.m = [np.zeros((self.K, n), dtype=self.dt) for n in self.numel] if (momentum != 0.0 or adam) else None
+        self.v = [np.zeros((self.K, n), dtype=self.dt) for n in self.numel] if adam else None
+        self.bpow = np.ones((self.L, self.K, 2), dtype=np.float64) if adam else None
+        self.tcount = np.zeros((self.L, self.K), dtype=np.int64) if adam else None
         self.w = np.full((self.L, self.K), 1.0 / self.K, dtype=np.float64)   # PAPER.md:106
 
     def layer_update(self, step, layer, g):
-        lr = float(np.float32(self.lr)) if self.dt == np.float64 else self.lr
-        mu = float(np.float32(self.mu)) if self.dt == np.float64 else self.mu
-        layer_update(self.x[layer], np.ascontiguousarray(g, dtype=np.float32),
-                     self.m[layer] if self.m is not None else None, self.w[layer],
-                     lr, mu, self.seed, step, layer, self.peer_mode, self.skip_prob,
-                     delay_replica=self.delay_replica, delay_rounds=self.delay_rounds)
+        g = np.ascontiguousarray(g, dtype=np.float32)
+        if self.optimizer == OPT_SGD and self.mix_mode == MIX_PUSHSUM and self.wd == 0.0:
+            lr = float(np.float32(self.lr)) if self.dt == np.float64 else self.lr
+            mu = float(np.float32(self.mu)) if self.dt == np.float64 else self.mu
+            layer_update(self.x[layer], g, self.m[layer] if self.m is not None else None, self.w[layer],
+                         lr, mu, self.seed, step, layer, self.peer_mode, self.skip_prob,
+                         delay_replica=self.delay_replica, delay_rounds=self.delay_rounds)
+            return
+        adam = self.optimizer == OPT_ADAMW
+        layer_update_ex(self.x[layer], g, self.m[layer] if self.m is not None else None,
+                        self.v[layer] if adam else None, self.w[layer],
+                        self.bpow[layer] if adam else None, self.tcount[layer] if adam else None,
+                        self.lr, self.mu, self.wd, self.beta1, self.beta2, self.eps, self.optimizer, self.mix_mode,
+                        self.seed, step, layer, self.peer_mode, self.skip_prob,
+                        delay_replica=self.delay_replica, delay_rounds=self.delay_rounds)
 
     def disagreement(self, weighted=False):
         """[L, K] squared distances to the (weighted) consensus, per layer."""

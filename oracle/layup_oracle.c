@@ -125,15 +125,65 @@ void oracle_schedule(uint64_t seed, int64_t step, int32_t L, int32_t K, int32_t 
       peer[(size_t)l * K + i] = active[i] ? oracle_peer(seed, step, l, i, K, peer_mode) : -1;
 }
 
+/* ---- options of the widened rule -----------------------
+ * optimizer 0: SGD, optional heavy-ball momentum mu (reading R8) and coupled weight decay
+ *              wd (the "weight_decay" row of PAPER.md:416-443, Tables A5/A6; PyTorch's SGD
+ *              convention d = g + wd*x, reading R21)
+ * optimizer 1: AdamW (PAPER.md:130 + Tables A7/A8 PAPER.md:469-491 "optimizer AdamW"),
+ *              decoupled decay, bias-corrected, PyTorch's convention (reading R21); the
+ *              moments m, v and the step count are local to the worker, never gossiped
+ * mix_mode 0 : push-sum fold, every colliding push applied (reading R3)
+ * mix_mode 1 : contention as the paper describes its own race ("the parameters
+ *              sent from one of the peers will be skipped", "not guaranteed that
+ *              all the weights for the push sum will be used"): of the pushes colliding on one
+ *              receiver only the LAST writer (highest sender index) lands, with its weight;
+ *              the skipped senders have already halved their weight and that mass is lost
+ *              (reading R22)
+ * mix_mode 2 : AD-PSGD-style symmetric pairwise averaging ("enforced symmetric
+ *              communication ... doubling the communication volume"): each active worker i, in
+ *              ascending index, atomically averages with its peer j: x_i, x_j <- (x_i+x_j)/2;
+ *              no push-sum weights (reading R23)
+ * All scalars are doubles holding fp32-representable values; the fp32 path narrows them. */
+typedef struct {
+  int32_t optimizer;
+  int32_t mix_mode;
+  double lr, mu, wd, beta1, beta2, eps;
+} oracle_opts;
+
+enum { OPT_SGD = 0, OPT_ADAMW = 1 };
+enum { MIX_PUSHSUM = 0, MIX_LOSSY = 1, MIX_SYMMETRIC = 2 };
+
+/* steps 1-2 of the header: mask, peers, halved weights.  Symmetric averaging carries no
+ * push-sum weight (R23), so nothing is halved there.                                     */
+static void draw_schedule(int32_t K, const double *w, uint64_t seed, int64_t step, int32_t layer,
+                          int32_t peer_mode, float skip_prob, int32_t delay_replica, int32_t delay_rounds,
+                          int32_t mix_mode, const int32_t *peer_in, const uint8_t *active_in,
+                          int32_t *peer, uint8_t *active, double *wh) {
+  for (int32_t i = 0; i < K; ++i) {
+    active[i] = active_in ? active_in[i]
+                          : (uint8_t)oracle_active_ex(seed, step, i, skip_prob, delay_replica, delay_rounds);
+    if (active[i] && K >= 2) {
+      peer[i] = peer_in ? peer_in[i] : oracle_peer(seed, step, layer, i, K, peer_mode);
+      wh[i] = mix_mode == MIX_SYMMETRIC ? w[i] : w[i] * 0.5;
+    } else {
+      peer[i] = -1;          /* inactive (or alone): no push, weight not halved */
+      wh[i] = w[i];
+    }
+  }
+}
+
 /* ---- one (step, layer) of the updater, fp32 state, fp64 push-sum weights ----
- * x, g, m : [K][n] row-major fp32 (m may be NULL when mu == 0);  w : [K] fp64.
- * peer_in/active_in: if non-NULL the schedule is taken from them instead of
- * being drawn (used by the brute-force tests to enumerate every schedule).
+ * x, g, m, v : [K][n] row-major fp32 (m NULL when unused: SGD with mu == 0; v NULL unless
+ * AdamW);  w : [K] fp64;  bpow : [K][2] fp64 = (beta1^t_i, beta2^t_i), 1.0 before the first
+ * step, AdamW only;  tcount : [K] steps worker i has taken on this layer, AdamW only.
+ * peer_in/active_in: if non-NULL the schedule is taken from them instead of being drawn
+ * (used by the brute-force tests to enumerate every schedule).
  * Returns 0, or -1 on allocation failure.                                    */
-int oracle_layer_update(int32_t K, int64_t n, float *x, const float *g, float *m, double *w,
-                        float lr, float mu, uint64_t seed, int64_t step, int32_t layer,
-                        int32_t peer_mode, float skip_prob, int32_t delay_replica, int32_t delay_rounds,
-                        const int32_t *peer_in, const uint8_t *active_in) {
+int oracle_layer_update_ex(int32_t K, int64_t n, float *x, const float *g, float *m, float *v, double *w,
+                           double *bpow, int64_t *tcount, const oracle_opts *o,
+                           uint64_t seed, int64_t step, int32_t layer,
+                           int32_t peer_mode, float skip_prob, int32_t delay_replica, int32_t delay_rounds,
+                           const int32_t *peer_in, const uint8_t *active_in) {
   int32_t *peer = (int32_t *)malloc(sizeof(int32_t) * (size_t)K);
   uint8_t *active = (uint8_t *)malloc((size_t)K);
   double *wh = (double *)malloc(sizeof(double) * (size_t)K);
@@ -143,73 +193,123 @@ int oracle_layer_update(int32_t K, int64_t n, float *x, const float *g, float *m
     free(peer); free(active); free(wh); free(y); free(acc);
     return -1;
   }
+  const float lr = (float)o->lr, mu = (float)o->mu, wd = (float)o->wd;
 
   /* 1. straggler mask; 2. peer choice and weight halving */
-  for (int32_t i = 0; i < K; ++i) {
-    active[i] = active_in ? active_in[i]
-                          : (uint8_t)oracle_active_ex(seed, step, i, skip_prob, delay_replica, delay_rounds);
-    if (active[i] && K >= 2) {
-      peer[i] = peer_in ? peer_in[i] : oracle_peer(seed, step, layer, i, K, peer_mode);
-      wh[i] = w[i] * 0.5;
-    } else {
-      peer[i] = -1;          /* inactive (or alone): no push, weight not halved */
-      wh[i] = w[i];
-    }
-  }
+  draw_schedule(K, w, seed, step, layer, peer_mode, skip_prob, delay_replica, delay_rounds, o->mix_mode,
+                peer_in, active_in, peer, active, wh);
 
   /* 3. local step on the current copy */
   for (int32_t i = 0; i < K; ++i) {
     float *xi = x + (size_t)i * n;
     const float *gi = g + (size_t)i * n;
     float *yi = y + (size_t)i * n;
-    if (active[i]) {
-      if (mu != 0.0f) {
-        float *mi = m + (size_t)i * n;
-        for (int64_t e = 0; e < n; ++e) {
-          const float mm = fmaf(mu, mi[e], gi[e]);   /* m <- mu*m + g        */
-          mi[e] = mm;
-          yi[e] = fmaf(-lr, mm, xi[e]);              /* y  = x - eta*m       */
-        }
-      } else {
-        for (int64_t e = 0; e < n; ++e) yi[e] = fmaf(-lr, gi[e], xi[e]);   /* y = x - eta*g */
+    if (!active[i]) {
+      for (int64_t e = 0; e < n; ++e) yi[e] = xi[e];
+    } else if (o->optimizer == OPT_ADAMW) {
+      /* AdamW (Loshchilov & Hutter), PyTorch's order of operations:
+       *   x <- x (1 - eta wd);  m <- b1 m + (1-b1) g;  v <- b2 v + (1-b2) g^2
+       *   x <- x - eta/(1-b1^t) * m / ( sqrt(v)/sqrt(1-b2^t) + eps )
+       * the per-step scalars come from fp64, rounded once to fp32                          */
+      float *mi = m + (size_t)i * n, *vi = v + (size_t)i * n;
+      const float b1 = (float)o->beta1, b2 = (float)o->beta2, eps = (float)o->eps;
+      const float omb1 = (float)(1.0 - (double)b1), omb2 = (float)(1.0 - (double)b2);
+      const float decay = (float)(1.0 - (double)lr * (double)wd);
+      bpow[2 * i + 0] *= (double)b1;                       /* beta1^t, t counted per worker  */
+      bpow[2 * i + 1] *= (double)b2;
+      tcount[i] += 1;
+      const float c1 = (float)((double)lr / (1.0 - bpow[2 * i + 0]));
+      const float c2 = (float)(1.0 / sqrt(1.0 - bpow[2 * i + 1]));
+      for (int64_t e = 0; e < n; ++e) {
+        const float xd = xi[e] * decay;
+        const float mm = fmaf(b1, mi[e], omb1 * gi[e]);
+        const float gg = gi[e] * gi[e];
+        const float vv = fmaf(b2, vi[e], omb2 * gg);
+        const float den = fmaf(sqrtf(vv), c2, eps);
+        mi[e] = mm;
+        vi[e] = vv;
+        yi[e] = fmaf(-c1, mm / den, xd);
       }
     } else {
-      for (int64_t e = 0; e < n; ++e) yi[e] = xi[e];
+      float *mi = mu != 0.0f ? m + (size_t)i * n : NULL;
+      for (int64_t e = 0; e < n; ++e) {
+        float d = gi[e];
+        if (wd != 0.0f) d = fmaf(wd, xi[e], d);      /* coupled decay: d = g + wd*x     */
+        if (mi) {
+          d = fmaf(mu, mi[e], d);                    /* m <- mu*m + d                   */
+          mi[e] = d;
+        }
+        yi[e] = fmaf(-lr, d, xi[e]);                 /* y  = x - eta*(m | d)            */
+      }
     }
   }
 
-  /* 4. peer update, once per sender of j in ascending sender index */
-  for (int32_t j = 0; j < K; ++j) {
-    double W = wh[j];
-    const float *yj = y + (size_t)j * n;
-    for (int64_t e = 0; e < n; ++e) acc[e] = yj[e];
+  if (o->mix_mode == MIX_SYMMETRIC) {
+    /* 4''. symmetric pairwise averaging, one atomic exchange per active worker, ascending i;
+     * each exchange sees the values the earlier ones left (a product of pairwise-averaging
+     * matrices, Lian et al. 2018).  Weights stay as they are.                              */
     for (int32_t i = 0; i < K; ++i) {
-      if (!(active[i] && peer[i] == j)) continue;
-      const float alpha = (float)(wh[i] / (W + wh[i]));   /* w_i/(w_i+w_j), one rounding */
-      const float *yi = y + (size_t)i * n;
+      if (!(active[i] && peer[i] >= 0)) continue;
+      float *yi = y + (size_t)i * n, *yj = y + (size_t)peer[i] * n;
       for (int64_t e = 0; e < n; ++e) {
-        const float d = yi[e] - acc[e];
-        acc[e] = fmaf(alpha, d, acc[e]);                  /* = (1-a)*x_j + a*x_i */
+        const float avg = 0.5f * (yi[e] + yj[e]);
+        yi[e] = avg;
+        yj[e] = avg;
       }
-      W = W + wh[i];                                      /* w_j <- w_j + w_i    */
     }
-    float *xj = x + (size_t)j * n;
-    for (int64_t e = 0; e < n; ++e) xj[e] = acc[e];
-    w[j] = W;
+    memcpy(x, y, sizeof(float) * (size_t)K * (size_t)n);
+  } else {
+    /* 4. peer update, once per sender of j in ascending sender index; under contention
+     * (MIX_LOSSY) only the last writer's push and weight land.                             */
+    for (int32_t j = 0; j < K; ++j) {
+      double W = wh[j];
+      const float *yj = y + (size_t)j * n;
+      int32_t last = -1;
+      for (int32_t i = 0; i < K; ++i)
+        if (active[i] && peer[i] == j) last = i;
+      for (int64_t e = 0; e < n; ++e) acc[e] = yj[e];
+      for (int32_t i = 0; i < K; ++i) {
+        if (!(active[i] && peer[i] == j)) continue;
+        if (o->mix_mode == MIX_LOSSY && i != last) continue;  /* overwritten: skipped       */
+        const float alpha = (float)(wh[i] / (W + wh[i]));   /* w_i/(w_i+w_j), one rounding */
+        const float *yi = y + (size_t)i * n;
+        for (int64_t e = 0; e < n; ++e) {
+          const float d = yi[e] - acc[e];
+          acc[e] = fmaf(alpha, d, acc[e]);                  /* = (1-a)*x_j + a*x_i */
+        }
+        W = W + wh[i];                                      /* w_j <- w_j + w_i    */
+      }
+      float *xj = x + (size_t)j * n;
+      for (int64_t e = 0; e < n; ++e) xj[e] = acc[e];
+      w[j] = W;
+    }
   }
 
   free(peer); free(active); free(wh); free(y); free(acc);
   return 0;
 }
 
+/* The rule of the header as first pinned: SGD (+ momentum), push-sum fold. */
+int oracle_layer_update(int32_t K, int64_t n, float *x, const float *g, float *m, double *w,
+                        float lr, float mu, uint64_t seed, int64_t step, int32_t layer,
+                        int32_t peer_mode, float skip_prob, int32_t delay_replica, int32_t delay_rounds,
+                        const int32_t *peer_in, const uint8_t *active_in) {
+  const oracle_opts o = {OPT_SGD, MIX_PUSHSUM, (double)lr, (double)mu, 0.0, 0.0, 0.0, 0.0};
+  return oracle_layer_update_ex(K, n, x, g, m, NULL, w, NULL, NULL, &o, seed, step, layer, peer_mode, skip_prob,
+                                delay_replica, delay_rounds, peer_in, active_in);
+}
+
 /* ---- fp64 shadow: same schedule, every value in double, and the mix written in
  * its closed form  x_j <- (wh_j y_j + sum_i wh_i y_i) / (wh_j + sum_i wh_i)
- * (PAPER.md:101 applied once per sender telescopes to this weighted centroid).
- * Used for the 100-round error bound and as an independent statement of step 4. */
-int oracle_layer_update_f64(int32_t K, int64_t n, double *x, const float *g, double *m, double *w,
-                            double lr, double mu, uint64_t seed, int64_t step, int32_t layer,
-                            int32_t peer_mode, float skip_prob, int32_t delay_replica, int32_t delay_rounds,
-                            const int32_t *peer_in, const uint8_t *active_in) {
+ * (PAPER.md:101 applied once per sender telescopes to this weighted centroid); AdamW's bias
+ * corrections from pow(beta, t) rather than running products.
+ * Used for the 100-round error bound and as an independent statement of steps 3-4. */
+int oracle_layer_update_ex_f64(int32_t K, int64_t n, double *x, const float *g, double *m, double *v, double *w,
+                               double *bpow, int64_t *tcount, const oracle_opts *o,
+                               uint64_t seed, int64_t step, int32_t layer,
+                               int32_t peer_mode, float skip_prob, int32_t delay_replica, int32_t delay_rounds,
+                               const int32_t *peer_in, const uint8_t *active_in) {
+  (void)bpow;
   int32_t *peer = (int32_t *)malloc(sizeof(int32_t) * (size_t)K);
   uint8_t *active = (uint8_t *)malloc((size_t)K);
   double *wh = (double *)malloc(sizeof(double) * (size_t)K);
@@ -218,52 +318,82 @@ int oracle_layer_update_f64(int32_t K, int64_t n, double *x, const float *g, dou
     free(peer); free(active); free(wh); free(y);
     return -1;
   }
+  const double lr = o->lr, mu = o->mu, wd = o->wd;
+  draw_schedule(K, w, seed, step, layer, peer_mode, skip_prob, delay_replica, delay_rounds, o->mix_mode,
+                peer_in, active_in, peer, active, wh);
   for (int32_t i = 0; i < K; ++i) {
-    active[i] = active_in ? active_in[i]
-                          : (uint8_t)oracle_active_ex(seed, step, i, skip_prob, delay_replica, delay_rounds);
-    if (active[i] && K >= 2) {
-      peer[i] = peer_in ? peer_in[i] : oracle_peer(seed, step, layer, i, K, peer_mode);
-      wh[i] = w[i] * 0.5;
-    } else {
-      peer[i] = -1;
-      wh[i] = w[i];
+    double bc1 = 1.0, bc2 = 1.0;
+    if (active[i] && o->optimizer == OPT_ADAMW) {
+      tcount[i] += 1;
+      bc1 = 1.0 - pow(o->beta1, (double)tcount[i]);
+      bc2 = 1.0 - pow(o->beta2, (double)tcount[i]);
     }
-  }
-  for (int32_t i = 0; i < K; ++i) {
     for (int64_t e = 0; e < n; ++e) {
-      const size_t o = (size_t)i * n + e;
-      if (active[i]) {
-        if (mu != 0.0) {
-          m[o] = mu * m[o] + (double)g[o];
-          y[o] = x[o] - lr * m[o];
-        } else {
-          y[o] = x[o] - lr * (double)g[o];
-        }
+      const size_t q = (size_t)i * n + e;
+      if (!active[i]) {
+        y[q] = x[q];
+      } else if (o->optimizer == OPT_ADAMW) {
+        const double gg = (double)g[q];
+        m[q] = o->beta1 * m[q] + (1.0 - o->beta1) * gg;
+        v[q] = o->beta2 * v[q] + (1.0 - o->beta2) * gg * gg;
+        y[q] = x[q] * (1.0 - lr * wd) - (lr / bc1) * m[q] / (sqrt(v[q]) / sqrt(bc2) + o->eps);
       } else {
-        y[o] = x[o];
+        double d = (double)g[q] + wd * x[q];
+        if (mu != 0.0) {
+          m[q] = mu * m[q] + d;
+          d = m[q];
+        }
+        y[q] = x[q] - lr * d;
       }
     }
   }
-  for (int32_t j = 0; j < K; ++j) {
-    double W = wh[j];
-    for (int32_t i = 0; i < K; ++i)
-      if (active[i] && peer[i] == j) W += wh[i];
-    for (int64_t e = 0; e < n; ++e) {
-      double s = wh[j] * y[(size_t)j * n + e];
-      for (int32_t i = 0; i < K; ++i)
-        if (active[i] && peer[i] == j) s += wh[i] * y[(size_t)i * n + e];
-      x[(size_t)j * n + e] = s / W;
+  if (o->mix_mode == MIX_SYMMETRIC) {
+    for (int32_t i = 0; i < K; ++i) {
+      if (!(active[i] && peer[i] >= 0)) continue;
+      for (int64_t e = 0; e < n; ++e) {
+        const double avg = (y[(size_t)i * n + e] + y[(size_t)peer[i] * n + e]) / 2.0;
+        y[(size_t)i * n + e] = avg;
+        y[(size_t)peer[i] * n + e] = avg;
+      }
     }
-  }
-  /* weights are updated after all receivers are done (wh is the pre-round view) */
-  for (int32_t j = 0; j < K; ++j) {
-    double W = wh[j];
-    for (int32_t i = 0; i < K; ++i)
-      if (active[i] && peer[i] == j) W = W + wh[i];
-    w[j] = W;
+    memcpy(x, y, sizeof(double) * (size_t)K * (size_t)n);
+  } else {
+    for (int32_t j = 0; j < K; ++j) {
+      int32_t last = -1;
+      for (int32_t i = 0; i < K; ++i)
+        if (active[i] && peer[i] == j) last = i;
+      double W = wh[j];
+      for (int32_t i = 0; i < K; ++i)
+        if (active[i] && peer[i] == j && (o->mix_mode == MIX_PUSHSUM || i == last)) W += wh[i];
+      for (int64_t e = 0; e < n; ++e) {
+        double s = wh[j] * y[(size_t)j * n + e];
+        for (int32_t i = 0; i < K; ++i)
+          if (active[i] && peer[i] == j && (o->mix_mode == MIX_PUSHSUM || i == last)) s += wh[i] * y[(size_t)i * n + e];
+        x[(size_t)j * n + e] = s / W;
+      }
+    }
+    /* weights are updated after all receivers are done (wh is the pre-round view) */
+    for (int32_t j = 0; j < K; ++j) {
+      int32_t last = -1;
+      for (int32_t i = 0; i < K; ++i)
+        if (active[i] && peer[i] == j) last = i;
+      double W = wh[j];
+      for (int32_t i = 0; i < K; ++i)
+        if (active[i] && peer[i] == j && (o->mix_mode == MIX_PUSHSUM || i == last)) W = W + wh[i];
+      w[j] = W;
+    }
   }
   free(peer); free(active); free(wh); free(y);
   return 0;
+}
+
+int oracle_layer_update_f64(int32_t K, int64_t n, double *x, const float *g, double *m, double *w,
+                            double lr, double mu, uint64_t seed, int64_t step, int32_t layer,
+                            int32_t peer_mode, float skip_prob, int32_t delay_replica, int32_t delay_rounds,
+                            const int32_t *peer_in, const uint8_t *active_in) {
+  const oracle_opts o = {OPT_SGD, MIX_PUSHSUM, lr, mu, 0.0, 0.0, 0.0, 0.0};
+  return oracle_layer_update_ex_f64(K, n, x, g, m, NULL, w, NULL, NULL, &o, seed, step, layer, peer_mode,
+                                    skip_prob, delay_replica, delay_rounds, peer_in, active_in);
 }
 
 /* ---- model disagreement (PAPER.md:389-395 Fig. A1; eq. (9)
