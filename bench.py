@@ -46,6 +46,10 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--optimizer", default="sgd", choices=["sgd", "adamw"],
+                    help="local step: the config's SGD(+momentum) [default, BASELINE.json] or AdamW (NEXT-3)")
+    ap.add_argument("--mix", default="pushsum", choices=["pushsum", "lossy", "symmetric"],
+                    help="mixer: push-sum fold [default, BASELINE.json], contention-lossy or symmetric (NEXT-4)")
     ap.add_argument("--mode", default="round", choices=["round", "layers"],
                     help="round: one persistent launch per step; layers: L per-layer launches on 4 streams")
     return ap.parse_args()
@@ -58,7 +62,22 @@ def get_workload(name):
         return synth.workload(name)
 
 
-def bytes_per_update(w):
+ADAMW = dict(weight_decay=0.0031235, beta1=0.9, beta2=0.95, eps=1e-8)   # PAPER.md:469-480 (GPT-2 medium row)
+MIXES = {"pushsum": 0, "lossy": 1, "symmetric": 2}
+
+
+def rule_kwargs(args):
+    """Keyword arguments shared by LayUp(...) and oracle.Oracle(...): optimiser and mixer."""
+    kw = dict(mix_mode=MIXES[args.mix])
+    if args.optimizer == "adamw":
+        kw.update(optimizer=1, **ADAMW)
+    return kw
+
+
+def bytes_per_update(w, args=None):
+    """read x, g; write x (+ read/write m (+ read/write v))."""
+    if args is not None and args.optimizer == "adamw":
+        return 28
     return 20 if w.momentum != 0.0 else 12
 
 
@@ -86,7 +105,7 @@ def committed_traffic(name):
 
 
 # ---- oracle sample (cpu_baseline and --impl reference) -------------------------------
-def oracle_sample(w, seconds, steps=None, warmup=0):
+def oracle_sample(w, seconds, steps=None, warmup=0, args=None):
     """Times oracle/ as it stands, single-threaded, on a bounded sample of the workload:
     the LAST layers of the layer list (output side first, as the path walks them) up to a
     budget of parameter updates per round."""
@@ -100,7 +119,9 @@ def oracle_sample(w, seconds, steps=None, warmup=0):
         tot += w.K * w.numel[l]
     layers = sorted(layers)
     sub = synth.shrink(w, [w.numel[l] for l in layers])
-    ref = oracle.Oracle(sub.numel, sub.K, sub.lr, sub.momentum, sub.seed, sub.peer_mode, sub.skip_prob)
+    mom = 0.0 if (args is not None and args.optimizer == "adamw") else sub.momentum
+    ref = oracle.Oracle(sub.numel, sub.K, sub.lr, mom, sub.seed, sub.peer_mode, sub.skip_prob,
+                        **(rule_kwargs(args) if args is not None else {}))
     xs, grads_fn = synth.host_state(sub)
     for l in range(sub.L):
         ref.x[l][:] = xs[l]
@@ -131,7 +152,7 @@ def oracle_sample(w, seconds, steps=None, warmup=0):
 def run_reference(args, w, rank, world):
     if rank != 0:
         return
-    ups, s_per_step, sample, _ = oracle_sample(w, args.cpu_seconds, steps=args.steps, warmup=min(args.warmup, 1))
+    ups, s_per_step, sample, _ = oracle_sample(w, args.cpu_seconds, steps=args.steps, warmup=min(args.warmup, 1), args=args)
     line = {
         "metric": METRIC, "value": ups, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": s_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
@@ -186,11 +207,11 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def algorithmic_bytes(w, lu, steps_range):
-    """12/20 B per active param-update, 8 B for an idle replica that receives."""
+def algorithmic_bytes(w, lu, steps_range, args=None):
+    """12/20/28 B per active param-update, 8 B for an idle replica that receives."""
     if w.skip_prob == 0.0:
         n = w.K * w.params_per_replica
-        return [bytes_per_update(w) * n] * len(steps_range), [n] * len(steps_range)
+        return [bytes_per_update(w, args) * n] * len(steps_range), [n] * len(steps_range)
     bts, ups = [], []
     numel = np.array(w.numel, dtype=np.float64)
     for s in steps_range:
@@ -198,7 +219,7 @@ def algorithmic_bytes(w, lu, steps_range):
         b = u = 0.0
         for i in range(w.K):
             if active[i]:
-                b += bytes_per_update(w) * numel.sum(); u += numel.sum()
+                b += bytes_per_update(w, args) * numel.sum(); u += numel.sum()
             else:
                 recv = np.array([(peer[l] == i).any() for l in range(w.L)])
                 b += 8 * numel[recv].sum()
@@ -232,7 +253,9 @@ def run_ours(args, w, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
-    lu = LayUp(w.K, w.numel, w.lr, w.momentum, w.seed + 1000 * rank, w.peer_mode, w.skip_prob, device=local_rank)
+    mom = 0.0 if args.optimizer == "adamw" else w.momentum
+    lu = LayUp(w.K, w.numel, w.lr, mom, w.seed + 1000 * rank, w.peer_mode, w.skip_prob, device=local_rank,
+               **rule_kwargs(args))
     for l in range(w.L):
         synth.fill_init_(w, l, lu.view(WHAT_X, l))
         synth.fill_grad_(w, 0, l, lu.view(WHAT_G, l), data_seed=w.seed + 1000 * rank)
@@ -275,7 +298,7 @@ def run_ours(args, w, rank, world, local_rank):
     lu.layup_profile(False)
     launches = lu.layup_launch_count() - launches0
     clocks = sampler.summary(t0, t1) if sampler else None
-    bts, ups = algorithmic_bytes(w, lu, range(first, first + args.steps))
+    bts, ups = algorithmic_bytes(w, lu, range(first, first + args.steps), args)
 
     ms, job_updates, job_bytes = reduce_over_ranks(dist, ms, sum(ups), sum(bts), torch.device("cuda", local_rank))
     value = job_updates / (ms * 1e-3)
@@ -287,7 +310,7 @@ def run_ours(args, w, rank, world, local_rank):
     bytes_per_launch = sum(bts) / max(n_k, 1)
     achieved = bytes_per_launch / (k_avg_ms * 1e-3) / 1e9 if k_avg_ms > 0 else 0.0
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": committed_traffic(w.name), "kernel": "layup_update_kernel",
+                "traffic": committed_traffic(w.name) if (args.optimizer, args.mix) == ("sgd", "pushsum") else None, "kernel": "layup_update_kernel",
                 "kernel_ms_avg": k_avg_ms, "kernel_launches": n_k, "algorithmic_bytes_per_launch": bytes_per_launch,
                 "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0}
 
@@ -315,7 +338,7 @@ def run_ours(args, w, rank, world, local_rank):
                 t = torch.tensor([e_s], device="cuda", dtype=torch.float64)
                 dist.all_reduce(t, op=dist.ReduceOp.MAX)
                 e_s = float(t.item())
-            _, e_ups = algorithmic_bytes(w, lu, range(e_first, e_first + args.e2e_steps))
+            _, e_ups = algorithmic_bytes(w, lu, range(e_first, e_first + args.e2e_steps), args)
             e2e = {"value": world * sum(e_ups) / e_s, "unit": UNIT, "h2d_bytes_per_step": 4 * total,
                    "d2h_bytes_per_step": 4 * total, "steps": args.e2e_steps, "ms_per_step": e_s / args.e2e_steps * 1e3,
                    "api": "layup_round_host (pinned host grads in, params out, layer-pipelined)"}
@@ -328,7 +351,7 @@ def run_ours(args, w, rank, world, local_rank):
         return
     cpu = None
     if not args.no_cpu_baseline and world == 1:
-        c_ups, _, sample, _ = oracle_sample(w, args.cpu_seconds)
+        c_ups, _, sample, _ = oracle_sample(w, args.cpu_seconds, args=args)
         cpu = {"value": c_ups, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
                "host_cores": os.cpu_count()}
     line = {
@@ -337,7 +360,7 @@ def run_ours(args, w, rank, world, local_rank):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "%s (%s)" % (w.name, w.note), "K": w.K, "L": w.L,
                    "params_per_replica": w.params_per_replica, "momentum": w.momentum, "lr": w.lr,
-                   "skip_prob": w.skip_prob, "mode": args.mode, "parallelism": "replicas only x%d" % world,
+                   "skip_prob": w.skip_prob, "mode": args.mode, "optimizer": args.optimizer, "mix": args.mix, "parallelism": "replicas only x%d" % world,
                    "l2": "inputs larger than L2" if job_bytes / args.steps / world > 4 * 126e6 else
                          "L2-resident working set (launch-latency bound, see DESIGN.md)"},
         "effective_hbm_gbs": eff_gbs, "frac_of_8TBs_nominal": eff_gbs / world / 8000.0,

@@ -24,7 +24,8 @@
  *  - There is no CPU fallback: without a CUDA device every launching call fails with
  *    LAYUP_ECUDA.
  *
- * Arena layout (DEVICE, fp32): three sections X | G | M (M only if momentum != 0), each
+ * Arena layout (DEVICE, fp32): sections X | G | M | V (M only if momentum != 0 or AdamW, V
+ * only for AdamW), each
  * `section_floats` long.  Inside a section layers are stored in order 0..L-1; layer l
  * holds its K replicas back to back, each slice padded to a multiple of 32 floats
  * (128 B):   addr(what, i, l, e) = arena + what*section + base[l] + i*pad[l] + e.
@@ -48,7 +49,17 @@ extern "C" {
 
 #define LAYUP_WHAT_X 0    /* parameters x^{i,l}                 */
 #define LAYUP_WHAT_G 1    /* gradient of this step   ("Backward pass")    */
-#define LAYUP_WHAT_M 2    /* momentum buffer, local to the worker (R8)      */
+#define LAYUP_WHAT_M 2    /* momentum buffer / AdamW first moment, local to the worker (R8, R21) */
+#define LAYUP_WHAT_V 3    /* AdamW second moment, local to the worker (R21)           */
+
+#define LAYUP_OPT_SGD   0 /* x <- x - eta*(g + wd*x), optional heavy-ball momentum */
+#define LAYUP_OPT_ADAMW 1 /* AdamW, PyTorch's convention (Tables A7/A8 469-491)        */
+
+#define LAYUP_MIX_PUSHSUM   0 /* push-sum fold, every colliding push applied (R3)      */
+#define LAYUP_MIX_LOSSY     1 /* contention: only the last writer's push and weight land
+                                 ("one of the peers will be skipped", 106; R22)         */
+#define LAYUP_MIX_SYMMETRIC 2 /* AD-PSGD-style pairwise averaging x_i,x_j <- (x_i+x_j)/2, ascending
+                                 worker index, no push-sum weights (R23)               */
 
 #define LAYUP_MAX_K 1024  /* replicas (workers) per ctx                               */
 
@@ -69,9 +80,16 @@ typedef struct {
   int32_t  delay_rounds;  /* ... completes one iteration every delay_rounds+1 rounds (active
                           only when (step+1) % (delay_rounds+1) == 0) and keeps receiving in
                           between; 0 = off.  ANDed with the skip_prob mask    */
+  int32_t  optimizer;  /* LAYUP_OPT_*: the local step of every worker                      */
+  int32_t  mix_mode;   /* LAYUP_MIX_*: how a push meets the peer's copy                    */
+  float    weight_decay; /* SGD: coupled, d = g + wd*x; AdamW: decoupled, x <- x(1-eta*wd)
+                          (the weight_decay rows of PAPER.md:416-443, 469-491)             */
+  float    beta1;      /* AdamW only: 0 <= beta1 < 1                                       */
+  float    beta2;      /* AdamW only: 0 <= beta2 < 1                                       */
+  float    eps;        /* AdamW only: >= 0                                                 */
 } layup_config;
 
-/* Bytes of device memory the arena needs for this config (X + G (+ M), padded). Pure. */
+/* Bytes of device memory the arena needs for this config (X + G (+ M (+ V)), padded). Pure. */
 int layup_arena_bytes(const layup_config *cfg, size_t *bytes);
 
 /* Create a ctx over a caller-owned DEVICE arena (128-B aligned, >= layup_arena_bytes).

@@ -12,7 +12,9 @@ import numpy as np
 import torch
 
 LAYUP_OK, LAYUP_EINVAL, LAYUP_ESTATE, LAYUP_ECUDA = 0, -1, -2, -3
-WHAT_X, WHAT_G, WHAT_M = 0, 1, 2
+WHAT_X, WHAT_G, WHAT_M, WHAT_V = 0, 1, 2, 3
+OPT_SGD, OPT_ADAMW = 0, 1
+MIX_PUSHSUM, MIX_LOSSY, MIX_SYMMETRIC = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "csrc", "liblayup.so")
@@ -29,7 +31,9 @@ class _Config(ctypes.Structure):
     _fields_ = [("K", ctypes.c_int32), ("L", ctypes.c_int32), ("numel", ctypes.POINTER(ctypes.c_int64)),
                 ("lr", ctypes.c_float), ("momentum", ctypes.c_float), ("seed", ctypes.c_uint64),
                 ("peer_mode", ctypes.c_int32), ("skip_prob", ctypes.c_float), ("device", ctypes.c_int32),
-                ("delay_replica", ctypes.c_int32), ("delay_rounds", ctypes.c_int32)]
+                ("delay_replica", ctypes.c_int32), ("delay_rounds", ctypes.c_int32),
+                ("optimizer", ctypes.c_int32), ("mix_mode", ctypes.c_int32), ("weight_decay", ctypes.c_float),
+                ("beta1", ctypes.c_float), ("beta2", ctypes.c_float), ("eps", ctypes.c_float)]
 
 
 EXPORTS = ["layup_arena_bytes", "layup_init", "layup_destroy", "layup_ptr", "layup_set_lr",
@@ -79,17 +83,19 @@ def _check(rc, ctx=None):
         raise LayUpError(rc, (load_library().layup_last_error(ctx) or b"").decode())
 
 
-def _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device, delay_replica=0, delay_rounds=0):
+def _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device, delay_replica=0, delay_rounds=0,
+            optimizer=OPT_SGD, mix_mode=MIX_PUSHSUM, weight_decay=0.0, beta1=0.9, beta2=0.999, eps=1e-8):
     arr = (ctypes.c_int64 * len(numel))(*[int(n) for n in numel])
     cfg = _Config(int(K), len(numel), arr, float(lr), float(momentum), int(seed), int(peer_mode),
-                  float(skip_prob), int(device), int(delay_replica), int(delay_rounds))
+                  float(skip_prob), int(device), int(delay_replica), int(delay_rounds),
+                  int(optimizer), int(mix_mode), float(weight_decay), float(beta1), float(beta2), float(eps))
     cfg._keep = arr
     return cfg
 
 
-def layup_arena_bytes(K, numel, momentum=0.0) -> int:
+def layup_arena_bytes(K, numel, momentum=0.0, optimizer=OPT_SGD) -> int:
     out = ctypes.c_size_t(0)
-    cfg = _config(K, numel, 0.0, momentum, 0, 0, 0.0, 0)
+    cfg = _config(K, numel, 0.0, momentum, 0, 0, 0.0, 0, optimizer=optimizer)
     _check(load_library().layup_arena_bytes(ctypes.byref(cfg), ctypes.byref(out)))
     return out.value
 
@@ -113,12 +119,16 @@ class LayUp:
 
     def __init__(self, K: int, numel: Sequence[int], lr: float, momentum: float = 0.0, seed: int = 0,
                  peer_mode: int = 0, skip_prob: float = 0.0, device: int = 0,
-                 delay_replica: int = 0, delay_rounds: int = 0):
+                 delay_replica: int = 0, delay_rounds: int = 0, optimizer: int = OPT_SGD,
+                 mix_mode: int = MIX_PUSHSUM, weight_decay: float = 0.0, beta1: float = 0.9, beta2: float = 0.999,
+                 eps: float = 1e-8):
         self.lib = load_library()
         self.K, self.L, self.numel = int(K), len(numel), [int(n) for n in numel]
         self.momentum = float(momentum)
         self.device = torch.device("cuda", device)
-        self._cfg = _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device, delay_replica, delay_rounds)
+        self.optimizer, self.mix_mode = int(optimizer), int(mix_mode)
+        self._cfg = _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device, delay_replica, delay_rounds,
+                            optimizer, mix_mode, weight_decay, beta1, beta2, eps)
         nbytes = ctypes.c_size_t(0)
         _check(self.lib.layup_arena_bytes(ctypes.byref(self._cfg), ctypes.byref(nbytes)))
         self.arena_bytes = nbytes.value

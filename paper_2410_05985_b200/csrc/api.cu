@@ -13,12 +13,15 @@
 #include "../../include/layup.h"
 #include "layup_internal.cuh"
 #include "philox.cuh"
+#include "rule.cuh"
 
 using namespace layup;
 
 struct layup_ctx {
   int32_t K = 0, L = 0, device = 0, peer_mode = 0;
   float lr = 0.f, mu = 0.f, skip_prob = 0.f;
+  int32_t optimizer = 0, mix_mode = 0, opt = 0, n_sections = 2;  // opt: OPT_* of rule.cuh
+  float wd = 0.f, beta1 = 0.f, beta2 = 0.f, eps = 0.f;
   uint32_t skip_thr = 0;
   uint64_t seed = 0;
   std::vector<LayerDesc> layers;          // host copy
@@ -36,7 +39,7 @@ struct layup_ctx {
   // device tables
   LayerDesc *d_layers = nullptr;
   long long *d_tile_prefix = nullptr;
-  double *d_w = nullptr;
+  double *d_w = nullptr, *d_bpow = nullptr;
   SchedTables t{};
   int32_t *d_peer_scratch = nullptr;
   unsigned char *d_active_scratch = nullptr;
@@ -82,9 +85,19 @@ static int check_config(const layup_config *cfg) {
   if (!(cfg->skip_prob >= 0.f && cfg->skip_prob <= 1.f)) return fail(nullptr, LAYUP_EINVAL, "skip_prob outside [0,1]");
   if (cfg->peer_mode != 0 && cfg->peer_mode != 1) return fail(nullptr, LAYUP_EINVAL, "peer_mode must be 0 or 1");
   if (!(cfg->momentum >= 0.f) || !(cfg->lr == cfg->lr)) return fail(nullptr, LAYUP_EINVAL, "lr / momentum invalid");
+  if (cfg->optimizer != LAYUP_OPT_SGD && cfg->optimizer != LAYUP_OPT_ADAMW) return fail(nullptr, LAYUP_EINVAL, "optimizer must be 0 (SGD) or 1 (AdamW)");
+  if (cfg->mix_mode < LAYUP_MIX_PUSHSUM || cfg->mix_mode > LAYUP_MIX_SYMMETRIC) return fail(nullptr, LAYUP_EINVAL, "mix_mode must be 0, 1 or 2");
+  if (!(cfg->weight_decay >= 0.f)) return fail(nullptr, LAYUP_EINVAL, "weight_decay invalid");
+  if (cfg->optimizer == LAYUP_OPT_ADAMW &&
+      !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f && cfg->beta2 >= 0.f && cfg->beta2 < 1.f && cfg->eps >= 0.f))
+    return fail(nullptr, LAYUP_EINVAL, "AdamW needs 0 <= beta1, beta2 < 1 and eps >= 0");
   if (cfg->delay_rounds < 0 || (cfg->delay_rounds > 0 && (cfg->delay_replica < 0 || cfg->delay_replica >= cfg->K)))
     return fail(nullptr, LAYUP_EINVAL, "delay_replica / delay_rounds invalid");
   return LAYUP_OK;
+}
+
+static int n_sections(const layup_config *cfg) {      // X, G (, M (, V))
+  return cfg->optimizer == LAYUP_OPT_ADAMW ? 4 : cfg->momentum != 0.f ? 3 : 2;
 }
 
 static long long section_floats(const layup_config *cfg) {
@@ -97,7 +110,7 @@ extern "C" int layup_arena_bytes(const layup_config *cfg, size_t *bytes) {
   int rc = check_config(cfg);
   if (rc) return rc;
   if (!bytes) return fail(nullptr, LAYUP_EINVAL, "bytes is NULL");
-  *bytes = (size_t)section_floats(cfg) * sizeof(float) * (cfg->momentum != 0.f ? 3 : 2);
+  *bytes = (size_t)section_floats(cfg) * sizeof(float) * n_sections(cfg);
   return LAYUP_OK;
 }
 
@@ -134,6 +147,10 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     ctx->skip_thr = cfg->skip_prob > 0.f ? (uint32_t)th : 0u;
   }
   ctx->delay_replica = cfg->delay_replica; ctx->delay_rounds = cfg->delay_rounds;
+  ctx->optimizer = cfg->optimizer; ctx->mix_mode = cfg->mix_mode; ctx->wd = cfg->weight_decay;
+  ctx->beta1 = cfg->beta1; ctx->beta2 = cfg->beta2; ctx->eps = cfg->eps;
+  ctx->n_sections = n_sections(cfg);
+  ctx->opt = cfg->optimizer == LAYUP_OPT_ADAMW ? OPT_ADAMW : cfg->momentum != 0.f ? OPT_SGD_MOM : OPT_SGD;
   ctx->arena = (float *)arena_dev;
   ctx->section = section_floats(cfg);
 
@@ -144,7 +161,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   const int items_target = std::max(256, items_env > 0 ? items_env : 1024);
   int C = 8;
   while ((long long)cfg->K * C * 2 <= items_target && C < 4096) C *= 2;
-  if (items_env <= 0 && cfg->momentum == 0.f && C < 32 && cfg->K <= 64) C = 32;
+  if (items_env <= 0 && ctx->n_sections == 2 && C < 32 && cfg->K <= 64) C = 32;
   ctx->C = C;
   ctx->log2C = 0;
   while ((1 << ctx->log2C) < C) ++ctx->log2C;
@@ -187,16 +204,16 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   ctx->launch_shape = env_int("LAYUP_PERSISTENT", -1);
   if (ctx->engine == 1) {
     // TMA-staged kernel stages x, g (, m) of the whole tile: fall back to the LDG kernel if it does not fit
-    const size_t need_smem = tma_smem_bytes(K, C, cfg->momentum != 0.f);
+    const size_t need_smem = tma_smem_bytes(K, C, ctx->opt);
     if (need_smem > prop.sharedMemPerBlockOptin) ctx->engine = 0;
     else ctx->smem = (int)need_smem;
   }
   if (ctx->engine == 1) {
     if (ctx->variant < 0 || ctx->variant >= tma_num_variants()) ctx->variant = 0;
-    CU_TRY_INIT(tma_kernel_setup(ctx->variant, ctx->smem, cfg->momentum != 0.f, &ctx->threads, &ctx->ctas_per_sm));
+    CU_TRY_INIT(tma_kernel_setup(ctx->variant, ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
   } else {
     if (ctx->variant < 0 || ctx->variant >= update_num_variants()) ctx->variant = 0;
-    CU_TRY_INIT(update_kernel_setup(ctx->variant, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
+    CU_TRY_INIT(update_kernel_setup(ctx->variant, ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
   }
   if (ctx->ctas_per_sm < 1) ctx->ctas_per_sm = 1;
   const int cap = env_int("LAYUP_CTAS_PER_SM", 0);
@@ -211,6 +228,15 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   CU_TRY_INIT(cudaMalloc(&ctx->t.senders, sizeof(int32_t) * L * K));
   CU_TRY_INIT(cudaMalloc(&ctx->t.alpha, sizeof(float) * L * K));
   CU_TRY_INIT(cudaMalloc(&ctx->t.flags, (size_t)L * K));
+  if (ctx->opt == OPT_ADAMW) {
+    CU_TRY_INIT(cudaMalloc(&ctx->t.c1, sizeof(float) * L * K));
+    CU_TRY_INIT(cudaMalloc(&ctx->t.c2, sizeof(float) * L * K));
+    CU_TRY_INIT(cudaMalloc(&ctx->d_bpow, sizeof(double) * 2 * L * K));
+    std::vector<double> ones((size_t)2 * L * K, 1.0);                    // beta^0
+    CU_TRY_INIT(cudaMemcpy(ctx->d_bpow, ones.data(), sizeof(double) * 2 * L * K, cudaMemcpyHostToDevice));
+    CU_TRY_INIT(cudaMemset(ctx->t.c1, 0, sizeof(float) * L * K));
+    CU_TRY_INIT(cudaMemset(ctx->t.c2, 0, sizeof(float) * L * K));
+  }
   CU_TRY_INIT(cudaMalloc(&ctx->d_peer_scratch, sizeof(int32_t) * L * K));
   CU_TRY_INIT(cudaMalloc(&ctx->d_active_scratch, (size_t)K));
   CU_TRY_INIT(cudaMalloc(&ctx->d_dist, sizeof(double) * L * K));
@@ -239,6 +265,7 @@ extern "C" int layup_destroy(layup_ctx *ctx) {
   for (auto &pr : ctx->prof_pool) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
   cudaFree(ctx->d_layers); cudaFree(ctx->d_tile_prefix); cudaFree(ctx->d_w);
   cudaFree(ctx->t.peer); cudaFree(ctx->t.recv_off); cudaFree(ctx->t.senders); cudaFree(ctx->t.alpha);
+  cudaFree(ctx->t.c1); cudaFree(ctx->t.c2); cudaFree(ctx->d_bpow);
   cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_active_scratch); cudaFree(ctx->d_dist);
   delete ctx;
   return LAYUP_OK;
@@ -246,7 +273,7 @@ extern "C" int layup_destroy(layup_ctx *ctx) {
 
 extern "C" int layup_ptr(layup_ctx *ctx, int32_t what, int32_t replica, int32_t layer, float **dptr, int64_t *numel) {
   if (!ctx || !dptr) return fail(ctx, LAYUP_EINVAL, "ctx or dptr is NULL");
-  if (what < 0 || what > 2 || (what == LAYUP_WHAT_M && ctx->mu == 0.f)) return fail(ctx, LAYUP_EINVAL, "what=%d not in this arena", what);
+  if (what < 0 || what >= ctx->n_sections) return fail(ctx, LAYUP_EINVAL, "what=%d not in this arena", what);
   if (replica < 0 || replica >= ctx->K || layer < 0 || layer >= ctx->L) return fail(ctx, LAYUP_EINVAL, "replica %d / layer %d out of range", replica, layer);
   const LayerDesc &d = ctx->layers[layer];
   *dptr = ctx->arena + (long long)what * ctx->section + d.base + (long long)replica * d.pad;
@@ -268,16 +295,24 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   sp.K = ctx->K; sp.L = L; sp.peer_mode = ctx->peer_mode;
   sp.delay_replica = ctx->delay_replica; sp.delay_rounds = ctx->delay_rounds;
   sp.layer_begin = L - pos_end;                       // layers [L-pos_end, L-pos_begin)
+  sp.mix_mode = ctx->mix_mode; sp.adamw = ctx->opt == OPT_ADAMW ? 1 : 0; sp.bpow = ctx->d_bpow;
+  sp.lr = (double)ctx->lr; sp.beta1 = (double)ctx->beta1; sp.beta2 = (double)ctx->beta2;
   CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
 
   UpdateParams up{};
   up.x = ctx->arena;
   up.g = ctx->arena + ctx->section;
-  up.m = ctx->mu != 0.f ? ctx->arena + 2 * ctx->section : nullptr;
+  up.m = ctx->n_sections >= 3 ? ctx->arena + 2 * ctx->section : nullptr;
+  up.v = ctx->n_sections >= 4 ? ctx->arena + 3 * ctx->section : nullptr;
   up.layers = ctx->d_layers; up.tile_prefix = ctx->d_tile_prefix; up.t = ctx->t;
   up.tile_begin = ctx->tile_prefix[pos_begin]; up.tile_end = ctx->tile_prefix[pos_end];
   up.K = ctx->K; up.L = L; up.C = ctx->C; up.log2C = ctx->log2C; up.pos_begin = pos_begin; up.pos_end = pos_end;
-  up.neg_lr = -ctx->lr; up.mu = ctx->mu; up.all_active = (ctx->skip_thr == 0u && ctx->delay_rounds == 0) ? 1 : 0;
+  up.s.neg_lr = -ctx->lr; up.s.mu = ctx->mu; up.s.wd = ctx->opt == OPT_ADAMW ? 0.f : ctx->wd;
+  up.s.b1 = ctx->beta1; up.s.b2 = ctx->beta2; up.s.eps = ctx->eps;
+  up.s.omb1 = (float)(1.0 - (double)ctx->beta1); up.s.omb2 = (float)(1.0 - (double)ctx->beta2);
+  up.s.decay = (float)(1.0 - (double)ctx->lr * (double)ctx->wd);          // AdamW: x <- x (1 - eta*wd)
+  up.opt = ctx->opt; up.symmetric = ctx->mix_mode == kMixSymmetric ? 1 : 0;
+  up.all_active = (ctx->skip_thr == 0u && ctx->delay_rounds == 0) ? 1 : 0;
   up.hints = ctx->hints;
   const long long tiles = up.tile_end - up.tile_begin;
   const long long resident = (long long)ctx->n_sm * ctx->ctas_per_sm;

@@ -22,6 +22,17 @@ struct SchedTables {
   int32_t *senders;         // [L*K]   senders of each receiver, ascending
   float *alpha;             // [L*K]   mixing coefficient of each push, same order
   unsigned char *flags;     // [L*K]   kFlagActive | kFlagRecv
+  float *c1, *c2;           // [L*K]   AdamW step scalars eta/(1-b1^t), 1/sqrt(1-b2^t) (else nullptr)
+};
+
+constexpr int kMixPushSum = 0;         // lossless push-sum fold (R3)
+constexpr int kMixLossy = 1;           // contention: only the last writer's push lands (R22)
+constexpr int kMixSymmetric = 2;       // AD-PSGD pairwise averaging (R23)
+
+// fp32 scalars of the local step (narrowed once on the host)
+struct StepScalars {
+  float neg_lr, mu, wd;                 // SGD: -eta, momentum, coupled weight decay
+  float b1, b2, omb1, omb2, eps, decay; // AdamW: betas, 1-betas, eps, 1 - eta*wd
 };
 
 struct SchedParams {
@@ -34,10 +45,14 @@ struct SchedParams {
   int32_t layer_begin;      // blockIdx.x + layer_begin = layer
   int32_t peer_mode;
   int32_t delay_replica, delay_rounds;   // deterministic straggler (0 rounds = off)
+  int32_t mix_mode;         // kMix*
+  int32_t adamw;            // 1: maintain bpow and emit c1, c2
+  double *bpow;             // [L*K*2] (beta1^t, beta2^t) per (layer, replica), AdamW only
+  double lr, beta1, beta2;  // fp32 values widened
 };
 
 struct UpdateParams {
-  float *x, *g, *m;                 // section bases (m == nullptr when momentum == 0)
+  float *x, *g, *m, *v;             // section bases (m / v == nullptr when the optimiser has none)
   const LayerDesc *layers;          // [L]
   const long long *tile_prefix;     // [L+1] by position; position p holds layer L-1-p
   SchedTables t;
@@ -45,7 +60,9 @@ struct UpdateParams {
   int32_t K, L;
   int32_t C, log2C;                 // float4 columns per tile (power of two)
   int32_t pos_begin, pos_end;       // positions covered by [tile_begin, tile_end)
-  float neg_lr, mu;
+  StepScalars s;
+  int32_t opt;                      // OPT_* of rule.cuh
+  int32_t symmetric;                // mix_mode == kMixSymmetric
   int32_t all_active;               // skip_prob == 0: every replica is active in every round
   int32_t hints;                    // bit 0: L2 evict-first on bulk loads; bit 1: streaming stores
 };
@@ -73,14 +90,14 @@ cudaError_t launch_disagreement(const float *x, const double *w, double *dist, i
                                 const PosTable &tab, int grid, int smem_bytes, cudaStream_t s);
 // update.cu
 int update_num_variants();
-cudaError_t update_kernel_setup(int variant, int smem_bytes, int *threads, int *ctas_per_sm);
+cudaError_t update_kernel_setup(int variant, int opt, bool symmetric, int smem_bytes, int *threads, int *ctas_per_sm);
 cudaError_t launch_update(const UpdateParams &p, int variant, bool persistent, int grid, int smem_bytes,
                           cudaStream_t s);
 size_t update_smem_bytes(int K, int C);
 // update_tma.cu -- TMA-bulk staged variants
 int tma_num_variants();
-size_t tma_smem_bytes(int K, int C, bool mom);
-cudaError_t tma_kernel_setup(int variant, int smem_bytes, bool mom, int *threads, int *ctas_per_sm);
+size_t tma_smem_bytes(int K, int C, int opt);
+cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_bytes, int *threads, int *ctas_per_sm);
 cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, int grid, int smem_bytes,
                               cudaStream_t s);
 

@@ -7,6 +7,12 @@
 //                w_j <- w_j + w_i"
 // Colliding pushes are folded in ascending sender index (R3): for receiver j,
 // alpha_k = wh_i / (W + wh_i), W <- W + wh_i, starting from W = wh_j.
+// Variant mixers: kMixLossy keeps only the last writer of every
+// receiver (R22) -- the update kernel is unchanged, it just sees a shorter
+// sender list; kMixSymmetric exchanges no weight (R23) and the update kernel
+// walks the peer table instead of a sender list.
+// AdamW (NEXT-3): the per-(layer, replica) bias corrections, from running products
+// beta^t kept in fp64, narrowed once: c1 = eta/(1-b1^t), c2 = 1/sqrt(1-b2^t).
 #include "layup_internal.cuh"
 #include "philox.cuh"
 
@@ -31,7 +37,15 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
     double wh = p.w[row + i];
     if (act && K >= 2) {
       peer = draw_peer(p.seed, p.step, p.peer_mode == 0 ? (uint32_t)layer : kNoLayer, i, K);
-      wh = wh * 0.5;                                             // w_i <- w_i / 2 (exact)
+      if (p.mix_mode != kMixSymmetric) wh = wh * 0.5;            // w_i <- w_i / 2 (exact)
+    }
+    if (p.adamw && act) {                                        // this worker takes its t-th step
+      const double p1 = __dmul_rn(p.bpow[2 * (row + i)], p.beta1);   // no contraction into 1 - p1
+      const double p2 = __dmul_rn(p.bpow[2 * (row + i) + 1], p.beta2);
+      p.bpow[2 * (row + i)] = p1;
+      p.bpow[2 * (row + i) + 1] = p2;
+      p.t.c1[row + i] = (float)(p.lr / (1.0 - p1));
+      p.t.c2[row + i] = (float)(1.0 / sqrt(1.0 - p2));
     }
     s_peer[i] = peer;
     s_wh[i] = wh;
@@ -42,7 +56,8 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
   int cnt = 0;
   if (i < K) {
     for (int s = 0; s < K; ++s) cnt += (s_peer[s] == i);
-    s_cnt[i] = cnt;
+    // entries of the sender list: all pushes, the last writer only, or none (symmetric)
+    s_cnt[i] = p.mix_mode == kMixPushSum ? cnt : p.mix_mode == kMixLossy ? (cnt > 0 ? 1 : 0) : 0;
   }
   __syncthreads();
   if (i == 0) {
@@ -55,15 +70,20 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
   if (i < K) {
     double W = s_wh[i];
     int k = s_off[i];
-    for (int s = 0; s < K; ++s) {
+    int last = -1;
+    if (p.mix_mode == kMixLossy)
+      for (int s = 0; s < K; ++s)
+        if (s_peer[s] == i) last = s;
+    for (int s = 0; s < K && p.mix_mode != kMixSymmetric; ++s) {
       if (s_peer[s] != i) continue;
+      if (p.mix_mode == kMixLossy && s != last) continue;        // overwritten: skipped
       const double ws = s_wh[s];
       p.t.senders[row + k] = s;
       p.t.alpha[row + k] = (float)(ws / (W + ws));               // one rounding to fp32
       W = W + ws;                                                // w_j <- w_j + w_i
       ++k;
     }
-    p.w[row + i] = W;
+    if (p.mix_mode != kMixSymmetric) p.w[row + i] = W;
     p.t.flags[row + i] = (unsigned char)((act ? kFlagActive : 0) | (cnt > 0 ? kFlagRecv : 0));
     p.t.recv_off[(size_t)layer * (K + 1) + i] = s_off[i];
     if (i == 0) p.t.recv_off[(size_t)layer * (K + 1) + K] = s_off[K];

@@ -5,9 +5,12 @@
 // copies (cp.async.bulk, the TMA engine; SASS UBLKCP) completing on one mbarrier, so the
 // whole tile (K*C*16 B * 3) is in flight per CTA without holding registers.  The local step
 // then runs out of shared memory, y overwrites x in place (the "send" is an on-chip read,
-// PAPER.md:101), m' goes straight to HBM, and after one CTA barrier every receiver folds
-// its senders and writes x once.  HBM traffic is unchanged: 12 B / 20 B per parameter update.
+// PAPER.md:101), m' (and AdamW's v') go straight to HBM, and after one CTA barrier every
+// receiver folds its senders and writes x once.  HBM traffic is unchanged: 12 B (SGD) / 20 B
+// (momentum) / 28 B (AdamW) per parameter update.  Template parameters: OPT = local optimiser
+// (rule.cuh), SYM = symmetric pairwise averaging instead of the push-sum fold.
 #include "layup_internal.cuh"
+#include "rule.cuh"
 
 namespace layup {
 
@@ -57,20 +60,25 @@ __device__ __forceinline__ uint64_t policy_evict_first() {
 __device__ __forceinline__ void st4(float *p, const float4 &v) { *reinterpret_cast<float4 *>(p) = v; }
 __device__ __forceinline__ void st4_cs(float *p, const float4 &v) { __stcs(reinterpret_cast<float4 *>(p), v); }
 
-template <bool MOM, int THREADS, int MINB>
+template <int OPT, bool SYM, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
     layup_update_tma(const __grid_constant__ UpdateParams p, const __grid_constant__ PosTable tab) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int NARR = OptTraits<OPT>::kArrays;
+  constexpr bool HAS_M = NARR >= 3, HAS_V = NARR >= 4;
   const int K = p.K, C = p.C, log2C = p.log2C, tid = threadIdx.x;
   const int n_items = K << log2C;
   float4 *xs = reinterpret_cast<float4 *>(smem_raw);                       // [K*C]  x, then y in place
   float4 *gs = xs + n_items;                                                // [K*C]
-  float4 *ms = MOM ? gs + n_items : gs;                                     // [K*C] (momentum only)
-  uint64_t *bar = reinterpret_cast<uint64_t *>((MOM ? ms : gs) + n_items);
+  float4 *ms = HAS_M ? gs + n_items : gs;                                   // [K*C] (momentum / Adam m)
+  float4 *vs = HAS_V ? ms + n_items : ms;                                   // [K*C] (Adam v)
+  uint64_t *bar = reinterpret_cast<uint64_t *>(xs + NARR * n_items);
   int *s_recv_off = reinterpret_cast<int *>(bar + 1);                       // [K+1]
-  int *s_senders = s_recv_off + (K + 1);                                    // [K]
+  int *s_senders = s_recv_off + (K + 1);                                    // [K]  (SYM: the peer table)
   float *s_alpha = reinterpret_cast<float *>(s_senders + K);                // [K]
-  unsigned char *s_flags = reinterpret_cast<unsigned char *>(s_alpha + K);  // [K]
+  float *s_c1 = s_alpha + K;                                                // [K]  (AdamW only)
+  float *s_c2 = s_c1 + (HAS_V ? K : 0);                                     // [K]  (AdamW only)
+  unsigned char *s_flags = reinterpret_cast<unsigned char *>(s_c2 + (HAS_V ? K : 0));  // [K]
 
   // which layer does this work item belong to: binary search in the parameter table
   const long long tile = blockIdx.x;
@@ -87,9 +95,9 @@ __global__ void __launch_bounds__(THREADS, MINB)
   const long long tile_off = tab.lay[lo].base + (col0 << 2);
   float *const xb = p.x + tile_off;
   const float *const gb = p.g + tile_off;
-  float *const mb = MOM ? p.m + tile_off : nullptr;
+  float *const mb = HAS_M ? p.m + tile_off : nullptr;
+  float *const vb = HAS_V ? p.v + tile_off : nullptr;
   const uint32_t chunk = (uint32_t)ncols * 16u;
-  constexpr int NARR = MOM ? 3 : 2;
 
   if (tid == 0) {
     mbar_init(bar, 1);
@@ -110,8 +118,8 @@ __global__ void __launch_bounds__(THREADS, MINB)
         if (!f || (a > 0 && !(f & kFlagActive))) continue;
       }
       const long long off = (long long)i * pad;
-      void *dst = a == 0 ? xs + (i << log2C) : a == 1 ? gs + (i << log2C) : ms + (i << log2C);
-      const float *src = a == 0 ? xb + off : a == 1 ? gb + off : mb + off;
+      void *dst = xs + a * n_items + (i << log2C);
+      const float *src = (a == 0 ? xb : a == 1 ? gb : a == 2 ? mb : vb) + off;
       if (p.hints & 1) bulk_g2s_ef(dst, src, chunk, bar, policy_evict_first());
       else bulk_g2s(dst, src, chunk, bar);
     }
@@ -122,9 +130,13 @@ __global__ void __launch_bounds__(THREADS, MINB)
   {
     const size_t row = (size_t)layer * K;
     for (int k = tid; k < K; k += THREADS) {
-      s_senders[k] = p.t.senders[row + k];
+      s_senders[k] = SYM ? p.t.peer[row + k] : p.t.senders[row + k];
       s_alpha[k] = p.t.alpha[row + k];
       s_flags[k] = p.t.flags[row + k];
+      if (HAS_V) {
+        s_c1[k] = p.t.c1[row + k];
+        s_c2[k] = p.t.c2[row + k];
+      }
     }
     for (int k = tid; k <= K; k += THREADS) s_recv_off[k] = p.t.recv_off[(size_t)layer * (K + 1) + k];
   }
@@ -147,57 +159,60 @@ __global__ void __launch_bounds__(THREADS, MINB)
   }
   mbar_wait(bar, 0);
 
-  // ---- phase 1: local step out of shared memory; y overwrites x in place, m' -> HBM
+  // ---- phase 1: local step out of shared memory; y overwrites x in place, m' (v') -> HBM
   for (int idx = tid; idx < n_items; idx += THREADS) {
     const int i = idx >> log2C, c = idx & (C - 1);
     if (c >= ncols) continue;
     if (!(s_flags[i] & kFlagActive)) continue;                              // idle replica: y = x already there
-    float4 y = xs[idx];
-    float4 d = gs[idx];
-    if (MOM) {
-      const float4 m = ms[idx];
-      d.x = __fmaf_rn(p.mu, m.x, d.x);
-      d.y = __fmaf_rn(p.mu, m.y, d.y);
-      d.z = __fmaf_rn(p.mu, m.z, d.z);
-      d.w = __fmaf_rn(p.mu, m.w, d.w);
-      if (p.hints & 2) st4_cs(mb + (long long)i * pad + (c << 2), d); else st4(mb + (long long)i * pad + (c << 2), d);
-    }
-    y.x = __fmaf_rn(p.neg_lr, d.x, y.x);
-    y.y = __fmaf_rn(p.neg_lr, d.y, y.y);
-    y.z = __fmaf_rn(p.neg_lr, d.z, y.z);
-    y.w = __fmaf_rn(p.neg_lr, d.w, y.w);
+    float4 m = HAS_M ? ms[idx] : float4{0.f, 0.f, 0.f, 0.f};
+    float4 v = HAS_V ? vs[idx] : float4{0.f, 0.f, 0.f, 0.f};
+    const float4 y = local_step4<OPT>(xs[idx], gs[idx], m, v, p.s, HAS_V ? s_c1[i] : 0.f, HAS_V ? s_c2[i] : 0.f);
+    const long long off = (long long)i * pad + (c << 2);
+    if (HAS_M) { if (p.hints & 2) st4_cs(mb + off, m); else st4(mb + off, m); }
+    if (HAS_V) { if (p.hints & 2) st4_cs(vb + off, v); else st4(vb + off, v); }
     xs[idx] = y;
   }
   __syncthreads();
 
-  // ---- phase 2: each receiver folds its senders in ascending order; x written once
-  for (int idx = tid; idx < n_items; idx += THREADS) {
-    const int i = idx >> log2C, c = idx & (C - 1);
-    if (c >= ncols) continue;
-    if (!s_flags[i]) continue;                                              // idle, no push received: 0 bytes
-    float4 acc = xs[idx];
-    const int k_end = s_recv_off[i + 1];
-    for (int k = s_recv_off[i]; k < k_end; ++k) {
-      const float a = s_alpha[k];
-      const float4 ys = xs[(s_senders[k] << log2C) + c];
-      acc.x = __fmaf_rn(a, __fsub_rn(ys.x, acc.x), acc.x);
-      acc.y = __fmaf_rn(a, __fsub_rn(ys.y, acc.y), acc.y);
-      acc.z = __fmaf_rn(a, __fsub_rn(ys.z, acc.z), acc.z);
-      acc.w = __fmaf_rn(a, __fsub_rn(ys.w, acc.w), acc.w);
+  if (SYM) {
+    // ---- phase 2 (symmetric): every scalar column runs the K exchanges in worker order
+    float *ysf = reinterpret_cast<float *>(xs);
+    for (int e = tid; e < (ncols << 2); e += THREADS) symmetric_column(ysf, C << 2, e, K, s_senders);
+    __syncthreads();
+    for (int idx = tid; idx < n_items; idx += THREADS) {
+      const int i = idx >> log2C, c = idx & (C - 1);
+      if (c >= ncols || !s_flags[i]) continue;                              // idle and nobody's peer: 0 bytes
+      st4(xb + (long long)i * pad + (c << 2), xs[idx]);
     }
-    if (p.hints & 2) st4_cs(xb + (long long)i * pad + (c << 2), acc); else st4(xb + (long long)i * pad + (c << 2), acc);
+  } else {
+    // ---- phase 2: each receiver folds its senders in ascending order; x written once
+    for (int idx = tid; idx < n_items; idx += THREADS) {
+      const int i = idx >> log2C, c = idx & (C - 1);
+      if (c >= ncols) continue;
+      if (!s_flags[i]) continue;                                            // idle, no push received: 0 bytes
+      float4 acc = xs[idx];
+      const int k_end = s_recv_off[i + 1];
+      for (int k = s_recv_off[i]; k < k_end; ++k) peer_update4(acc, xs[(s_senders[k] << log2C) + c], s_alpha[k]);
+      if (p.hints & 2) st4_cs(xb + (long long)i * pad + (c << 2), acc); else st4(xb + (long long)i * pad + (c << 2), acc);
+    }
   }
 }
 
 using TmaFn = void (*)(const UpdateParams, const PosTable);
 struct TmaVariant {
   int threads, minb;
-  TmaFn fn[2];
+  TmaFn fn[3][2];   // [OPT][SYM]
 };
-#define LAYUP_TMA_VARIANT(T, MB) TmaVariant{T, MB, {layup_update_tma<false, T, MB>, layup_update_tma<true, T, MB>}}
+#define LAYUP_TMA_VARIANT(T, MB)                                                                              \
+  TmaVariant {                                                                                                \
+    T, MB, {                                                                                                  \
+      {layup_update_tma<OPT_SGD, false, T, MB>, layup_update_tma<OPT_SGD, true, T, MB>},                      \
+          {layup_update_tma<OPT_SGD_MOM, false, T, MB>, layup_update_tma<OPT_SGD_MOM, true, T, MB>},          \
+          {layup_update_tma<OPT_ADAMW, false, T, MB>, layup_update_tma<OPT_ADAMW, true, T, MB>},              \
+    }                                                                                                         \
+  }
 const TmaVariant kTma[] = {
     LAYUP_TMA_VARIANT(256, 4), LAYUP_TMA_VARIANT(128, 8), LAYUP_TMA_VARIANT(512, 2), LAYUP_TMA_VARIANT(256, 2),
-    LAYUP_TMA_VARIANT(128, 4), LAYUP_TMA_VARIANT(256, 8), LAYUP_TMA_VARIANT(64, 16),
 };
 constexpr int kNumTma = sizeof(kTma) / sizeof(kTma[0]);
 
@@ -205,14 +220,16 @@ constexpr int kNumTma = sizeof(kTma) / sizeof(kTma[0]);
 
 int tma_num_variants() { return kNumTma; }
 
-size_t tma_smem_bytes(int K, int C, bool mom) {
-  return (size_t)K * C * sizeof(float4) * (mom ? 3 : 2) + 8 + sizeof(int) * (2 * (size_t)K + 1) + sizeof(float) * K + (size_t)K;
+size_t tma_smem_bytes(int K, int C, int opt) {
+  const int narr = opt == OPT_ADAMW ? 4 : opt == OPT_SGD_MOM ? 3 : 2;
+  return (size_t)K * C * sizeof(float4) * narr + 8 + sizeof(int) * (2 * (size_t)K + 1) +
+         sizeof(float) * K * (opt == OPT_ADAMW ? 3 : 1) + (size_t)K;
 }
 
-cudaError_t tma_kernel_setup(int variant, int smem_bytes, bool mom, int *threads, int *ctas_per_sm) {
-  if (variant < 0 || variant >= kNumTma) return cudaErrorInvalidValue;
+cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_bytes, int *threads, int *ctas_per_sm) {
+  if (variant < 0 || variant >= kNumTma || opt < 0 || opt > 2) return cudaErrorInvalidValue;
   const TmaVariant &v = kTma[variant];
-  TmaFn f = v.fn[mom ? 1 : 0];
+  TmaFn f = v.fn[opt][symmetric ? 1 : 0];
   cudaError_t e;
   if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
@@ -226,7 +243,7 @@ cudaError_t tma_kernel_setup(int variant, int smem_bytes, bool mom, int *threads
 cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, int grid, int smem_bytes,
                               cudaStream_t s) {
   const TmaVariant &v = kTma[variant];
-  v.fn[p.m != nullptr ? 1 : 0]<<<grid, v.threads, smem_bytes, s>>>(p, tab);
+  v.fn[p.opt][p.symmetric ? 1 : 0]<<<grid, v.threads, smem_bytes, s>>>(p, tab);
   return cudaGetLastError();
 }
 

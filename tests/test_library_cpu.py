@@ -45,6 +45,7 @@ def test_arena_bytes_layout():
     # slices padded to 32 floats, X|G(|M) sections
     assert pkg.layup_arena_bytes(4, [1, 31, 32, 33], 0.0) == 4 * (32 + 32 + 32 + 64) * 4 * 2
     assert pkg.layup_arena_bytes(4, [1, 31, 32, 33], 0.9) == 4 * (32 + 32 + 32 + 64) * 4 * 3
+    assert pkg.layup_arena_bytes(4, [1, 31, 32, 33], 0.0, optimizer=pkg.OPT_ADAMW) == 4 * (32 + 32 + 32 + 64) * 4 * 4
     with pytest.raises(pkg.LayUpError) as e:
         pkg.layup_arena_bytes(0, [10])
     assert e.value.code == pkg.LAYUP_EINVAL

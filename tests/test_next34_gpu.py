@@ -1,0 +1,216 @@
+"""GPU parity for SURVEY.md 8(f) NEXT-3 (AdamW, coupled weight decay) and NEXT-4 (contention-lossy
+and symmetric mixers): the CUDA path through the C-ABI against the oracle on the same seeded
+bytes, every round, bit-exact schedule and weights, parameters and optimiser state within 1e-6
+(and, the two sides sharing the order of fp32 operations, 0 ulp)."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from _util import REL_TOL_100, REL_TOL_ROUND, max_ulp, rel_err
+from paper_2410_05985_b200 import (LAYUP_EINVAL, MIX_LOSSY, MIX_PUSHSUM, MIX_SYMMETRIC, OPT_ADAMW, OPT_SGD, WHAT_G,
+                                   WHAT_M, WHAT_V, WHAT_X, LayUp, LayUpError)
+
+pytestmark = pytest.mark.gpu
+
+ADAM = dict(weight_decay=0.0031235, beta1=0.9, beta2=0.95, eps=1e-8)       # PAPER.md:469-480 + GPT-2 betas
+
+
+def _pair(K, numel, lr, mu, seed, skip, opt, mix, peer_mode=0, shadow=False, **kw):
+    lu = LayUp(K, numel, lr, mu, seed, peer_mode, skip, optimizer=opt, mix_mode=mix, **kw)
+    ref = oracle.Oracle(numel, K, lr, mu, seed, peer_mode, skip, optimizer=opt, mix_mode=mix, **kw)
+    sh = oracle.Oracle(numel, K, lr, mu, seed, peer_mode, skip, optimizer=opt, mix_mode=mix, f64=True, **kw) if shadow else None
+    w = synth.Workload("t", K, tuple(numel), lr, mu, 0, seed, grad_std=1e-3, heavy_frac=0.01, heavy_scale=100.0)
+    for l in range(len(numel)):
+        synth.fill_init_(w, l, lu.view(WHAT_X, l))
+        x0 = lu.view(WHAT_X, l).cpu().numpy()
+        ref.x[l][:] = x0
+        if sh is not None:
+            sh.x[l][:] = x0
+    return w, lu, ref, sh
+
+
+def _run(w, lu, ref, sh, rounds, expect_zero_ulp=True):
+    worst_ulp = 0
+    for step in range(rounds):
+        grads = []
+        for l in range(w.L):
+            synth.fill_grad_(w, step, l, lu.view(WHAT_G, l))
+            grads.append(lu.view(WHAT_G, l).cpu().numpy())
+        lu.layup_round(step)
+        lu.layup_sync()
+        ref.round(step, grads)
+        if sh is not None:
+            sh.round(step, grads)
+        for l in range(w.L):
+            pairs = [(WHAT_X, ref.x[l])]
+            if ref.m is not None:
+                pairs.append((WHAT_M, ref.m[l]))
+            if ref.v is not None:
+                pairs.append((WHAT_V, ref.v[l]))
+            for what, want in pairs:
+                got = lu.view(what, l).cpu().numpy()
+                assert rel_err(got, want) <= REL_TOL_ROUND, (step, l, what, rel_err(got, want))
+                worst_ulp = max(worst_ulp, max_ulp(got, want))
+        assert np.array_equal(lu.layup_weights(), ref.w), step
+    if sh is not None:
+        for l in range(w.L):
+            assert rel_err(lu.view(WHAT_X, l).cpu().numpy(), sh.x[l]) <= REL_TOL_100
+    if expect_zero_ulp:
+        assert worst_ulp == 0, worst_ulp
+    return worst_ulp
+
+
+NUMEL = [515 * 40, 19 * 40, 80, 40 * 120 + 120, 1, 33, 4097]     # several tiles, ragged tails, tiny layers
+
+
+@pytest.mark.parametrize("K,skip", [(1, 0.0), (2, 0.0), (3, 0.25), (8, 0.0), (16, 0.25), (33, 0.1), (64, 0.0)])
+def test_adamw_parity_every_round(K, skip):
+    w, lu, ref, sh = _pair(K, NUMEL, 7.5249e-4, 0.0, 11 + K, skip, OPT_ADAMW, MIX_PUSHSUM, shadow=True, **ADAM)
+    _run(w, lu, ref, sh, 12)
+    lu.close()
+
+
+@pytest.mark.parametrize("mu,wd", [(0.0, 0.005), (0.9, 0.0001), (0.9, 0.014)])
+def test_sgd_weight_decay_parity(mu, wd):
+    w, lu, ref, sh = _pair(8, NUMEL, 0.035, mu, 5, 0.25, OPT_SGD, MIX_PUSHSUM, shadow=True, weight_decay=wd)
+    _run(w, lu, ref, sh, 12)
+    lu.close()
+
+
+@pytest.mark.parametrize("K,skip,mu", [(2, 0.0, 0.0), (4, 0.0, 0.9), (8, 0.25, 0.9), (16, 0.0, 0.0), (64, 0.1, 0.0)])
+@pytest.mark.parametrize("mix", [MIX_LOSSY, MIX_SYMMETRIC])
+def test_variant_mixers_parity(K, skip, mu, mix):
+    w, lu, ref, sh = _pair(K, NUMEL, 0.01, mu, 3 * K + mix, skip, OPT_SGD, mix, shadow=True)
+    _run(w, lu, ref, sh, 15)
+    wts = lu.layup_weights()
+    if mix == MIX_SYMMETRIC:
+        assert np.array_equal(wts, np.full_like(wts, 1.0 / K))               # no push-sum weight moves
+    elif K > 2:
+        assert (wts.sum(axis=1) < 1.0).any()                                 # contention lost some mass
+    lu.close()
+
+
+@pytest.mark.parametrize("mix", [MIX_LOSSY, MIX_SYMMETRIC])
+@pytest.mark.parametrize("peer_mode", [0, 1])
+def test_adamw_with_variant_mixers(mix, peer_mode):
+    w, lu, ref, sh = _pair(8, NUMEL, 1e-3, 0.0, 21, 0.2, OPT_ADAMW, mix, peer_mode=peer_mode, shadow=True, **ADAM)
+    _run(w, lu, ref, sh, 10)
+    lu.close()
+
+
+def test_symmetric_k2_exact_average_and_mean_conservation_on_device():
+    K, n = 2, 4099
+    lu = LayUp(K, [n], 0.0, 0.0, 9, mix_mode=MIX_SYMMETRIC)
+    rng = np.random.default_rng(0)
+    x = (rng.integers(-2**16, 2**16, size=(K, n)) / 1024.0).astype(np.float32)
+    lu.view(WHAT_X, 0).copy_(torch.from_numpy(x))
+    lu.layup_round(0)
+    lu.layup_sync()
+    got = lu.view(WHAT_X, 0).cpu().numpy()
+    want = ((x[0].astype(np.float64) + x[1]) / 2).astype(np.float32)
+    assert np.array_equal(got[0], want) and np.array_equal(got[1], want)
+    lu.close()
+    K = 16
+    lu = LayUp(K, [n], 0.0, 0.0, 9, mix_mode=MIX_SYMMETRIC)
+    x = rng.normal(0, 1, (K, n)).astype(np.float32)
+    lu.view(WHAT_X, 0).copy_(torch.from_numpy(x))
+    mean0 = x.astype(np.float64).mean(axis=0)
+    prev = lu.layup_disagreement().sum()
+    for t in range(30):
+        lu.layup_round(t)
+        d = lu.layup_disagreement().sum()
+        assert d <= prev * (1 + 1e-6)
+        prev = d
+    got = lu.view(WHAT_X, 0).cpu().numpy().astype(np.float64)
+    np.testing.assert_allclose(got.mean(axis=0), mean0, atol=4 * K * 2**-24 * 30)
+    lu.close()
+
+
+def test_layer_calls_equal_round_for_adamw():
+    """layup_layer_update on streams, output layer first, == layup_round bit for bit (AdamW state included)."""
+    K = 8
+    outs = []
+    for mode in ("round", "layers"):
+        w, lu, ref, _ = _pair(K, NUMEL, 1e-3, 0.0, 4, 0.25, OPT_ADAMW, MIX_PUSHSUM, **ADAM)
+        streams = [torch.cuda.Stream() for _ in range(3)]
+        for step in range(5):
+            for l in range(w.L):
+                synth.fill_grad_(w, step, l, lu.view(WHAT_G, l))
+            torch.cuda.synchronize()
+            if mode == "round":
+                lu.layup_round(step)
+            else:
+                for k, l in enumerate(reversed(range(w.L))):
+                    lu.layup_layer_update(step, l, streams[k % 3])
+            lu.layup_sync()
+        outs.append([lu.view(what, l).cpu().numpy().copy() for l in range(w.L) for what in (WHAT_X, WHAT_M, WHAT_V)])
+        lu.close()
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("opt,mix,K", [(OPT_ADAMW, MIX_PUSHSUM, 8), (OPT_ADAMW, MIX_SYMMETRIC, 8), (OPT_SGD, MIX_SYMMETRIC, 16),
+                                       (OPT_ADAMW, MIX_PUSHSUM, 500)])
+def test_ldg_engine_covers_the_widened_rule(opt, mix, K, monkeypatch):
+    """The LDG kernels (large K, or LAYUP_ENGINE=0) implement the same optimisers and mixers.
+    K = 500 with AdamW does not fit the TMA staging and takes the LDG engine by itself."""
+    if K < 100:
+        monkeypatch.setenv("LAYUP_ENGINE", "0")
+    kw = ADAM if opt == OPT_ADAMW else {}
+    numel = NUMEL if K < 100 else [4097, 33, 800]
+    w, lu, ref, _ = _pair(K, numel, 1e-3, 0.0, 8, 0.2, opt, mix, **kw)
+    _run(w, lu, ref, None, 6)
+    lu.close()
+
+
+def test_adamw_full_size_sampled_parity():
+    """configs[1] shapes (K = 8 GPT-2-small) with AdamW at full size, sampled columns (as
+    test_parity_gpu.test_full_size_sampled_parity): 28 B per parameter update."""
+    wl = synth.workload("gpt2s_k8")
+    free, _ = torch.cuda.mem_get_info()
+    need = wl.K * sum((n + 31) // 32 * 32 for n in wl.numel) * 4 * 4
+    if need + (8 << 30) > free:
+        pytest.skip("needs %.1f GB of HBM" % (need / 2**30))
+    lu = LayUp(wl.K, wl.numel, wl.lr, 0.0, wl.seed, optimizer=OPT_ADAMW, **ADAM)
+    rng = np.random.default_rng(1)
+    from test_parity_gpu import _sample_columns
+    cols = [torch.from_numpy(_sample_columns(n, max(8, 1024 // wl.K), rng)).cuda() for n in wl.numel]
+    ref = oracle.Oracle([int(c.numel()) for c in cols], wl.K, wl.lr, 0.0, wl.seed, optimizer=OPT_ADAMW, **ADAM)
+    for l in range(wl.L):
+        synth.fill_init_(wl, l, lu.view(WHAT_X, l))
+        ref.x[l][:] = lu.view(WHAT_X, l)[:, cols[l]].cpu().numpy()
+    for step in range(3):
+        grads = []
+        for l in range(wl.L):
+            synth.fill_grad_(wl, step, l, lu.view(WHAT_G, l))
+            grads.append(lu.view(WHAT_G, l)[:, cols[l]].cpu().numpy())
+        lu.layup_round(step)
+        lu.layup_sync()
+        ref.round(step, grads)
+        for l in range(wl.L):
+            for what, want in ((WHAT_X, ref.x[l]), (WHAT_M, ref.m[l]), (WHAT_V, ref.v[l])):
+                got = lu.view(what, l)[:, cols[l]].cpu().numpy()
+                assert rel_err(got, want) <= REL_TOL_ROUND and max_ulp(got, want) == 0, (step, l, what)
+        assert np.array_equal(lu.layup_weights(), ref.w)
+    lu.close()
+    del lu
+    torch.cuda.empty_cache()
+
+
+def test_argument_errors_of_the_new_fields():
+    for kw in (dict(optimizer=2), dict(mix_mode=3), dict(weight_decay=-1.0), dict(optimizer=OPT_ADAMW, beta1=1.0),
+               dict(optimizer=OPT_ADAMW, eps=-1e-8)):
+        with pytest.raises(LayUpError) as e:
+            LayUp(4, [100], 0.1, **kw)
+        assert e.value.code == LAYUP_EINVAL
+    lu = LayUp(4, [100], 0.1)
+    with pytest.raises(LayUpError):
+        lu.ptr(WHAT_V, 0, 0)                      # no V section without AdamW
+    lu.close()
+    lu = LayUp(4, [100], 0.1, optimizer=OPT_ADAMW)
+    assert lu.view(WHAT_V, 0).shape == (4, 100) and lu.view(WHAT_M, 0).shape == (4, 100)
+    lu.close()
