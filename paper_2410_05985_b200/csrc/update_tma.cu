@@ -57,6 +57,19 @@ __device__ __forceinline__ uint64_t policy_evict_first() {
   return pol;
 }
 
+// shared::cta -> global bulk copy (TMA store), bytes % 16 == 0; completion tracked by bulk groups
+__device__ __forceinline__ void bulk_s2g(void *dst_gmem, const void *src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)),
+               "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit_wait_read() {
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+  asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+// generic-proxy writes to shared memory -> visible to the async proxy (TMA) before it reads them
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 __device__ __forceinline__ void st4(float *p, const float4 &v) { *reinterpret_cast<float4 *>(p) = v; }
 __device__ __forceinline__ void st4_cs(float *p, const float4 &v) { __stcs(reinterpret_cast<float4 *>(p), v); }
 
@@ -160,6 +173,7 @@ __global__ void __launch_bounds__(THREADS, MINB)
   mbar_wait(bar, 0);
 
   // ---- phase 1: local step out of shared memory; y overwrites x in place, m' (v') -> HBM
+  const bool bulk_out = (p.hints & 4) != 0;     // outputs leave through TMA bulk stores instead of STG
   for (int idx = tid; idx < n_items; idx += THREADS) {
     const int i = idx >> log2C, c = idx & (C - 1);
     if (c >= ncols) continue;
@@ -168,11 +182,26 @@ __global__ void __launch_bounds__(THREADS, MINB)
     float4 v = HAS_V ? vs[idx] : float4{0.f, 0.f, 0.f, 0.f};
     const float4 y = local_step4<OPT>(xs[idx], gs[idx], m, v, p.s, HAS_V ? s_c1[i] : 0.f, HAS_V ? s_c2[i] : 0.f);
     const long long off = (long long)i * pad + (c << 2);
-    if (HAS_M) { if (p.hints & 2) st4_cs(mb + off, m); else st4(mb + off, m); }
-    if (HAS_V) { if (p.hints & 2) st4_cs(vb + off, v); else st4(vb + off, v); }
+    if (bulk_out) {
+      if (HAS_M) ms[idx] = m;
+      if (HAS_V) vs[idx] = v;
+    } else {
+      if (HAS_M) { if (p.hints & 2) st4_cs(mb + off, m); else st4(mb + off, m); }
+      if (HAS_V) { if (p.hints & 2) st4_cs(vb + off, v); else st4(vb + off, v); }
+    }
     xs[idx] = y;
   }
+  if (bulk_out && HAS_M) fence_proxy_async();
   __syncthreads();
+  if (bulk_out && HAS_M) {
+    // m' (v') of every active replica: one bulk store per (replica, array), spread like the loads
+    constexpr int NOUT = HAS_M ? NARR - 2 : 1;
+    for (int c = slot0; c < K * NOUT; c += THREADS) {
+      const int i = c / NOUT, a = 2 + (c - i * NOUT);
+      if (!(s_flags[i] & kFlagActive)) continue;
+      bulk_s2g((a == 2 ? mb : vb) + (long long)i * pad, xs + a * n_items + (i << log2C), chunk);
+    }
+  }
 
   if (SYM) {
     // ---- phase 2 (symmetric): every scalar column runs the K exchanges in worker order
@@ -193,9 +222,18 @@ __global__ void __launch_bounds__(THREADS, MINB)
       float4 acc = xs[idx];
       const int k_end = s_recv_off[i + 1];
       for (int k = s_recv_off[i]; k < k_end; ++k) peer_update4(acc, xs[(s_senders[k] << log2C) + c], s_alpha[k]);
-      if (p.hints & 2) st4_cs(xb + (long long)i * pad + (c << 2), acc); else st4(xb + (long long)i * pad + (c << 2), acc);
+      if (bulk_out) gs[idx] = acc;                                          // g is dead: its tile carries x out
+      else if (p.hints & 2) st4_cs(xb + (long long)i * pad + (c << 2), acc);
+      else st4(xb + (long long)i * pad + (c << 2), acc);
+    }
+    if (bulk_out) {
+      fence_proxy_async();
+      __syncthreads();
+      for (int i = slot0; i < K; i += THREADS)
+        if (s_flags[i]) bulk_s2g(xb + (long long)i * pad, gs + (i << log2C), chunk);
     }
   }
+  if (bulk_out) bulk_commit_wait_read();   // shared memory must outlive the stores' reads
 }
 
 using TmaFn = void (*)(const UpdateParams, const PosTable);
