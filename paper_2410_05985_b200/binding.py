@@ -106,8 +106,13 @@ def layup_peer(seed, step, layer, replica, K) -> int:
     return out.value
 
 
-def _stream_handle(stream) -> Optional[int]:
+_raw_stream = getattr(torch._C, "_cuda_getCurrentRawStream", None)
+
+
+def _stream_handle(stream, device_index=None) -> Optional[int]:
     if stream is None:
+        if _raw_stream is not None and device_index is not None:
+            return _raw_stream(device_index) or None
         return torch.cuda.current_stream().cuda_stream or None
     if isinstance(stream, torch.cuda.Stream):
         return stream.cuda_stream or None
@@ -166,10 +171,10 @@ class LayUp:
         _check(self.lib.layup_set_lr(self.ctx, lr), self.ctx)
 
     def layup_layer_update(self, step: int, layer: int, stream=None):
-        _check(self.lib.layup_layer_update(self.ctx, step, layer, _stream_handle(stream)), self.ctx)
+        _check(self.lib.layup_layer_update(self.ctx, step, layer, _stream_handle(stream, self.device.index)), self.ctx)
 
     def layup_round(self, step: int, stream=None):
-        _check(self.lib.layup_round(self.ctx, step, _stream_handle(stream)), self.ctx)
+        _check(self.lib.layup_round(self.ctx, step, _stream_handle(stream, self.device.index)), self.ctx)
 
     def layup_round_host(self, step: int, g_host: torch.Tensor, x_host: Optional[torch.Tensor]):
         _check(self.lib.layup_round_host(self.ctx, step, g_host.data_ptr(),

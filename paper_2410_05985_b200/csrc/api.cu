@@ -1,5 +1,6 @@
 // C-ABI of liblayup (include/layup.h): argument checking, arena layout, step bookkeeping,
 // launches.  Every step of the path itself runs in the kernels of schedule.cu / update.cu.
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -32,7 +33,6 @@ struct layup_ctx {
   int C = 0, log2C = 0, smem = 0, ctas_per_sm = 1, n_sm = 1;
   int variant = 0, threads = 256, launch_shape = -1;   // launch_shape: -1 auto, 0 grouped, 1 persistent
   int engine = 1;                                      // 1: TMA-staged kernel, 0: LDG kernel
-  int hints = 0;                                       // cache-hint bits of UpdateParams::hints
   int32_t delay_replica = 0, delay_rounds = 0;
   int diag_C = 0, diag_log2C = 0, diag_smem = 0, diag_ctas = 1;
   double *d_dist = nullptr;
@@ -41,7 +41,10 @@ struct layup_ctx {
   long long *d_tile_prefix = nullptr;
   double *d_w = nullptr, *d_bpow = nullptr;
   SchedTables t{};
-  int32_t *d_peer_scratch = nullptr;
+  int32_t *d_peer_scratch = nullptr, *d_ticket = nullptr;
+  void *d_tmaps = nullptr;                // [n_sections][L] CUtensorMap: 2-D tiled view [K][pad] of every layer section
+  bool fused_ok = false;                  // the single-launch path exists for this ctx (K, engine, variant)
+  long long fused_max_tiles = 0;          // ... and is taken by launches of at most this many work items
   unsigned char *d_active_scratch = nullptr;
   // bookkeeping
   std::vector<cudaStream_t> streams;      // every stream launched on
@@ -162,6 +165,16 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   int C = 8;
   while ((long long)cfg->K * C * 2 <= items_target && C < 4096) C *= 2;
   if (items_env <= 0 && ctx->n_sections == 2 && C < 32 && cfg->K <= 64) C = 32;
+  if (items_env <= 0) {
+    // a whole round of fewer work items than ~4 per SM is latency bound: smaller tiles, more CTAs
+    // (B200: 148 SMs; chunks stay >= 256 B per replica)
+    auto round_tiles = [&](int c) {
+      long long t = 0;
+      for (int l = 0; l < cfg->L; ++l) t += (pad32(cfg->numel[l]) / 4 + c - 1) / c;
+      return t;
+    };
+    while (C > 16 && round_tiles(C) < 4 * 148) C /= 2;
+  }
   ctx->C = C;
   ctx->log2C = 0;
   while ((1 << ctx->log2C) < C) ++ctx->log2C;
@@ -199,23 +212,28 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     return bail(LAYUP_EINVAL);
   }
   ctx->engine = env_int("LAYUP_ENGINE", 1);
-  ctx->hints = env_int("LAYUP_HINTS", 0);
   ctx->variant = env_int("LAYUP_VARIANT", 0);
   ctx->launch_shape = env_int("LAYUP_PERSISTENT", -1);
   if (ctx->engine == 1) {
     // TMA-staged kernel stages x, g (, m) of the whole tile: fall back to the LDG kernel if it does not fit
-    const size_t need_smem = tma_smem_bytes(K, C, ctx->opt);
-    if (need_smem > prop.sharedMemPerBlockOptin) ctx->engine = 0;
+    if (ctx->variant < 0 || ctx->variant >= tma_num_variants()) ctx->variant = 0;
+    ctx->fused_ok = K <= kFusedMaxK && tma_has_fused(ctx->variant) && env_int("LAYUP_FUSED", 1) != 0;
+    const size_t need_smem = tma_smem_bytes(K, C, ctx->opt, ctx->fused_ok);
+    if (need_smem > prop.sharedMemPerBlockOptin) { ctx->engine = 0; ctx->fused_ok = false; }
     else ctx->smem = (int)need_smem;
   }
   if (ctx->engine == 1) {
-    if (ctx->variant < 0 || ctx->variant >= tma_num_variants()) ctx->variant = 0;
     CU_TRY_INIT(tma_kernel_setup(ctx->variant, ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
   } else {
     if (ctx->variant < 0 || ctx->variant >= update_num_variants()) ctx->variant = 0;
     CU_TRY_INIT(update_kernel_setup(ctx->variant, ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
   }
   if (ctx->ctas_per_sm < 1) ctx->ctas_per_sm = 1;
+  // launches of up to this many work items are launch-latency bound: one fused launch beats two
+  // (measured on B200 with every launch fused: K = 8 ties, K = 16 loses 8 %, K = 64 loses 45 % on
+  //  HBM-sized rounds -- the redundant schedule stage is only free while the launch is latency bound)
+  const int waves = env_int("LAYUP_FUSED_WAVES", 4);
+  ctx->fused_max_tiles = (long long)waves * ctx->n_sm * ctx->ctas_per_sm;
   const int cap = env_int("LAYUP_CTAS_PER_SM", 0);
   if (cap > 0 && cap < ctx->ctas_per_sm) ctx->ctas_per_sm = cap;
 
@@ -238,8 +256,40 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     CU_TRY_INIT(cudaMemset(ctx->t.c2, 0, sizeof(float) * L * K));
   }
   CU_TRY_INIT(cudaMalloc(&ctx->d_peer_scratch, sizeof(int32_t) * L * K));
+  CU_TRY_INIT(cudaMalloc(&ctx->d_ticket, sizeof(int32_t) * L));
+  CU_TRY_INIT(cudaMemset(ctx->d_ticket, 0, sizeof(int32_t) * L));
   CU_TRY_INIT(cudaMalloc(&ctx->d_active_scratch, (size_t)K));
   CU_TRY_INIT(cudaMalloc(&ctx->d_dist, sizeof(double) * L * K));
+  if (ctx->engine == 1 && env_int("LAYUP_TMA2D", 1) != 0 && K <= 256 && C * 4 <= 256) {
+    // One tensor map per (section, layer): rank 2, inner dim = the padded slice, outer dim = the K
+    // replicas (stride = pad), box = [K][C*4 floats], no swizzle, zero fill past the slice end.
+    typedef CUresult (*EncodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    bool ok = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+              qres == cudaDriverEntryPointSuccess && fn != nullptr;
+    std::vector<CUtensorMap> maps((size_t)ctx->n_sections * L);
+    for (int a = 0; ok && a < ctx->n_sections; ++a)
+      for (int l = 0; ok && l < L; ++l) {
+        const LayerDesc &d = ctx->layers[l];
+        if (d.pad >= (1ll << 31)) { ok = false; break; }                  // box coordinates are int32
+        const cuuint64_t gdim[2] = {(cuuint64_t)d.pad, (cuuint64_t)K};
+        const cuuint64_t gstride[1] = {(cuuint64_t)d.pad * sizeof(float)};
+        const cuuint32_t box[2] = {(cuuint32_t)(C * 4), (cuuint32_t)K};
+        const cuuint32_t estride[2] = {1, 1};
+        void *base_ptr = ctx->arena + (long long)a * ctx->section + d.base;
+        ok = ((EncodeTiled)fn)(&maps[(size_t)a * L + l], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base_ptr, gdim, gstride, box,
+                               estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+      }
+    cudaGetLastError();
+    if (ok) {
+      CU_TRY_INIT(cudaMalloc(&ctx->d_tmaps, sizeof(CUtensorMap) * maps.size()));
+      CU_TRY_INIT(cudaMemcpy(ctx->d_tmaps, maps.data(), sizeof(CUtensorMap) * maps.size(), cudaMemcpyHostToDevice));
+    }
+  }
   CU_TRY_INIT(cudaMemcpy(ctx->d_layers, ctx->layers.data(), sizeof(LayerDesc) * L, cudaMemcpyHostToDevice));
   CU_TRY_INIT(cudaMemcpy(ctx->d_tile_prefix, ctx->tile_prefix.data(), sizeof(long long) * (L + 1), cudaMemcpyHostToDevice));
   std::vector<double> w0((size_t)L * K, 1.0 / (double)K);              // PAPER.md:106  w_i = 1/M
@@ -266,7 +316,7 @@ extern "C" int layup_destroy(layup_ctx *ctx) {
   cudaFree(ctx->d_layers); cudaFree(ctx->d_tile_prefix); cudaFree(ctx->d_w);
   cudaFree(ctx->t.peer); cudaFree(ctx->t.recv_off); cudaFree(ctx->t.senders); cudaFree(ctx->t.alpha);
   cudaFree(ctx->t.c1); cudaFree(ctx->t.c2); cudaFree(ctx->d_bpow);
-  cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_active_scratch); cudaFree(ctx->d_dist);
+  cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_ticket); cudaFree(ctx->d_tmaps); cudaFree(ctx->d_active_scratch); cudaFree(ctx->d_dist);
   delete ctx;
   return LAYUP_OK;
 }
@@ -297,7 +347,9 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   sp.layer_begin = L - pos_end;                       // layers [L-pos_end, L-pos_begin)
   sp.mix_mode = ctx->mix_mode; sp.adamw = ctx->opt == OPT_ADAMW ? 1 : 0; sp.bpow = ctx->d_bpow;
   sp.lr = (double)ctx->lr; sp.beta1 = (double)ctx->beta1; sp.beta2 = (double)ctx->beta2;
-  CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
+  sp.ticket = ctx->d_ticket;
+  const bool fused = ctx->fused_ok && ctx->tile_prefix[pos_end] - ctx->tile_prefix[pos_begin] <= ctx->fused_max_tiles;
+  if (!fused) CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
 
   UpdateParams up{};
   up.x = ctx->arena;
@@ -313,7 +365,8 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   up.s.decay = (float)(1.0 - (double)ctx->lr * (double)ctx->wd);          // AdamW: x <- x (1 - eta*wd)
   up.opt = ctx->opt; up.symmetric = ctx->mix_mode == kMixSymmetric ? 1 : 0;
   up.all_active = (ctx->skip_thr == 0u && ctx->delay_rounds == 0) ? 1 : 0;
-  up.hints = ctx->hints;
+  up.sched = sp;
+  up.tmaps = ctx->d_tmaps;
   const long long tiles = up.tile_end - up.tile_begin;
   const long long resident = (long long)ctx->n_sm * ctx->ctas_per_sm;
 
@@ -339,7 +392,7 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
       if (n == 0) return fail(ctx, LAYUP_EINVAL, "layer %d has more than 2^31 tiles", L - 1 - q0);
       tab.prefix[n] = ctx->tile_prefix[q0 + n] - t0;
       tab.n = n;
-      CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, (int)tab.prefix[n], ctx->smem, s));
+      CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, fused, (int)tab.prefix[n], ctx->smem, s));
       q0 += n;
       ++n_launch;
     }
@@ -354,7 +407,7 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
     CU_TRY(ctx, cudaEventRecord(ev.second, s));
     ctx->prof_pending.push_back(ev);
   }
-  ctx->launches += 1 + n_launch;
+  ctx->launches += (fused ? 0 : 1) + n_launch;
   note_stream(ctx, s);
   return LAYUP_OK;
 }

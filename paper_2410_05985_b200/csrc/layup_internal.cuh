@@ -49,7 +49,9 @@ struct SchedParams {
   int32_t adamw;            // 1: maintain bpow and emit c1, c2
   double *bpow;             // [L*K*2] (beta1^t, beta2^t) per (layer, replica), AdamW only
   double lr, beta1, beta2;  // fp32 values widened
+  int32_t *ticket;          // [L] zero between launches; fused single-launch path only (update_tma.cu)
 };
+constexpr int kFusedMaxK = 64;         // the in-kernel schedule stage is O(K) per thread
 
 struct UpdateParams {
   float *x, *g, *m, *v;             // section bases (m / v == nullptr when the optimiser has none)
@@ -64,7 +66,8 @@ struct UpdateParams {
   int32_t opt;                      // OPT_* of rule.cuh
   int32_t symmetric;                // mix_mode == kMixSymmetric
   int32_t all_active;               // skip_prob == 0: every replica is active in every round
-  int32_t hints;                    // bit 0: L2 evict-first on bulk loads; bit 1: streaming stores
+  SchedParams sched;                // fused single-launch path: the schedule stage's inputs
+  const void *tmaps;                // [n_sections][L] CUtensorMap (128 B each) of the layer sections, or nullptr
 };
 
 // Work-list table of one launch, passed by value in the kernel parameters (constant bank):
@@ -96,9 +99,10 @@ cudaError_t launch_update(const UpdateParams &p, int variant, bool persistent, i
 size_t update_smem_bytes(int K, int C);
 // update_tma.cu -- TMA-bulk staged variants
 int tma_num_variants();
-size_t tma_smem_bytes(int K, int C, int opt);
+size_t tma_smem_bytes(int K, int C, int opt, bool fused);
+bool tma_has_fused(int variant);
 cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_bytes, int *threads, int *ctas_per_sm);
-cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, int grid, int smem_bytes,
-                              cudaStream_t s);
+cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, int grid,
+                              int smem_bytes, cudaStream_t s);
 
 }  // namespace layup

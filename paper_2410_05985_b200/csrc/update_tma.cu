@@ -10,6 +10,7 @@
 // (momentum) / 28 B (AdamW) per parameter update.  Template parameters: OPT = local optimiser
 // (rule.cuh), SYM = symmetric pairwise averaging instead of the push-sum fold.
 #include "layup_internal.cuh"
+#include "philox.cuh"
 #include "rule.cuh"
 
 namespace layup {
@@ -42,38 +43,25 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
                : "memory");
 }
 
-// same copy with an L2 evict-first policy: every byte of the arena is touched once per round
-__device__ __forceinline__ void bulk_g2s_ef(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar,
-                                            uint64_t policy) {
+// 2-D tiled TMA load: ONE instruction brings the [K rows x C*4 floats] box of a layer section
+// (rows = replicas, row stride = the padded slice) into shared memory as a dense [K][C*4] tile;
+// columns past the end of the slice are zero-filled.  tmap: a CUtensorMap in global memory.
+__device__ __forceinline__ void tma_load_2d(void *dst_smem, const void *tmap, int c0, int c1, uint64_t *bar) {
   asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
           smem_u32(dst_smem)),
-      "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+      "l"(tmap), "r"(c0), "r"(c1), "r"(smem_u32(bar))
       : "memory");
 }
-__device__ __forceinline__ uint64_t policy_evict_first() {
-  uint64_t pol;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-  return pol;
-}
-
-// shared::cta -> global bulk copy (TMA store), bytes % 16 == 0; completion tracked by bulk groups
-__device__ __forceinline__ void bulk_s2g(void *dst_gmem, const void *src_smem, uint32_t bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)),
-               "r"(bytes)
-               : "memory");
-}
-__device__ __forceinline__ void bulk_commit_wait_read() {
-  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-  asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-}
-// generic-proxy writes to shared memory -> visible to the async proxy (TMA) before it reads them
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 __device__ __forceinline__ void st4(float *p, const float4 &v) { *reinterpret_cast<float4 *>(p) = v; }
-__device__ __forceinline__ void st4_cs(float *p, const float4 &v) { __stcs(reinterpret_cast<float4 *>(p), v); }
 
-template <int OPT, bool SYM, int THREADS, int MINB>
+// FUSED: the schedule stage (schedule.cu) runs inside this kernel -- ONE launch per round or
+// per layer event instead of two.  Every CTA of a layer recomputes that layer's O(K) schedule in
+// shared memory from the same inputs (seed, step, w, beta powers), so all CTAs agree bit for bit;
+// the CTA that is LAST to have read the state (a ticket per layer) writes the new w / beta powers
+// back in place.  Used for launches of few tiles (launch-latency bound) and K <= kFusedMaxK.
+template <int OPT, bool SYM, bool FUSED, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
     layup_update_tma(const __grid_constant__ UpdateParams p, const __grid_constant__ PosTable tab) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -86,9 +74,14 @@ __global__ void __launch_bounds__(THREADS, MINB)
   float4 *ms = HAS_M ? gs + n_items : gs;                                   // [K*C] (momentum / Adam m)
   float4 *vs = HAS_V ? ms + n_items : ms;                                   // [K*C] (Adam v)
   uint64_t *bar = reinterpret_cast<uint64_t *>(xs + NARR * n_items);
-  int *s_recv_off = reinterpret_cast<int *>(bar + 1);                       // [K+1]
-  int *s_senders = s_recv_off + (K + 1);                                    // [K]  (SYM: the peer table)
-  float *s_alpha = reinterpret_cast<float *>(s_senders + K);                // [K]
+  double *s_wh = reinterpret_cast<double *>(bar + 1);                       // [K]  FUSED only: halved weights
+  double *s_wnew = s_wh + (FUSED ? K : 0);                                  // [K]  FUSED only: w after the round
+  double *s_bp = s_wnew + (FUSED ? K : 0);                                  // [2K] FUSED + AdamW: new beta powers
+  int *s_begin = reinterpret_cast<int *>(s_bp + (FUSED && HAS_V ? 2 * K : 0));   // [K] first sender slot
+  int *s_cnt = s_begin + K;                                                 // [K]  senders of each receiver
+  int *s_senders = s_cnt + K;                                               // [K]  (SYM: the peer table)
+  int *s_peer = s_senders + K;                                              // [K]  FUSED only
+  float *s_alpha = reinterpret_cast<float *>(s_peer + (FUSED ? K : 0));     // [K]
   float *s_c1 = s_alpha + K;                                                // [K]  (AdamW only)
   float *s_c2 = s_c1 + (HAS_V ? K : 0);                                     // [K]  (AdamW only)
   unsigned char *s_flags = reinterpret_cast<unsigned char *>(s_c2 + (HAS_V ? K : 0));  // [K]
@@ -112,10 +105,19 @@ __global__ void __launch_bounds__(THREADS, MINB)
   float *const vb = HAS_V ? p.v + tile_off : nullptr;
   const uint32_t chunk = (uint32_t)ncols * 16u;
 
+  const bool boxed = p.all_active && p.tmaps != nullptr;   // whole-tile 2-D TMA loads, one per array
   if (tid == 0) {
     mbar_init(bar, 1);
     // no straggler this round: every replica is active, the byte count is known up front
-    if (p.all_active) mbar_expect_tx(bar, (uint32_t)K * NARR * chunk);
+    if (boxed) {
+      mbar_expect_tx(bar, (uint32_t)n_items * 16u * NARR);                  // full boxes, zero fill included
+      const unsigned char *tm = reinterpret_cast<const unsigned char *>(p.tmaps);
+#pragma unroll
+      for (int a = 0; a < NARR; ++a)
+        tma_load_2d(xs + a * n_items, tm + ((size_t)a * p.L + layer) * 128, (int)(col0 << 2), 0, bar);
+    } else if (p.all_active) {
+      mbar_expect_tx(bar, (uint32_t)K * NARR * chunk);
+    }
   }
   __syncthreads();   // mbarrier visible
 
@@ -133,27 +135,101 @@ __global__ void __launch_bounds__(THREADS, MINB)
       const long long off = (long long)i * pad;
       void *dst = xs + a * n_items + (i << log2C);
       const float *src = (a == 0 ? xb : a == 1 ? gb : a == 2 ? mb : vb) + off;
-      if (p.hints & 1) bulk_g2s_ef(dst, src, chunk, bar, policy_evict_first());
-      else bulk_g2s(dst, src, chunk, bar);
+      bulk_g2s(dst, src, chunk, bar);
     }
   };
-  if (p.all_active) issue_copies(false);
+  if (p.all_active && !boxed) issue_copies(false);
 
   // this layer's schedule -> shared memory (overlaps the bulk copies when all replicas are active)
-  {
+  int ticket = -1;
+  if (FUSED) {
+    // the schedule stage itself (same arithmetic as layup_schedule_kernel, K <= THREADS)
+    const SchedParams &q = p.sched;
+    const size_t row = (size_t)layer * K;
+    bool act = false;
+    if (tid < K) {
+      const int i = tid;
+      act = draw_active(q.seed, q.step, i, q.skip_thr, q.delay_replica, q.delay_rounds);
+      int peer = -1;
+      double wh = q.w[row + i];
+      if (act && K >= 2) {
+        peer = draw_peer(q.seed, q.step, q.peer_mode == 0 ? (uint32_t)layer : kNoLayer, i, K);
+        if (!SYM) wh = wh * 0.5;                                 // w_i <- w_i / 2 (exact)
+      }
+      if (HAS_V) {
+        double p1 = q.bpow[2 * (row + i)], p2 = q.bpow[2 * (row + i) + 1];
+        if (act) {
+          p1 = __dmul_rn(p1, q.beta1);
+          p2 = __dmul_rn(p2, q.beta2);
+          s_c1[i] = (float)(q.lr / (1.0 - p1));
+          s_c2[i] = (float)(1.0 / sqrt(1.0 - p2));
+        }
+        s_bp[2 * i] = p1;
+        s_bp[2 * i + 1] = p2;
+      }
+      s_peer[i] = peer;
+      s_wh[i] = wh;
+    }
+    __syncthreads();
+    if (tid < K) {
+      const int j = tid;
+      int cnt = 0, below = 0, last = -1;
+      for (int sdr = 0; sdr < K; ++sdr) {
+        const int pr = s_peer[sdr];
+        cnt += (pr == j);
+        below += (pr >= 0 && pr < j);
+        if (pr == j) last = sdr;
+      }
+      double W = s_wh[j];
+      int n_list = 0;
+      if (SYM) {
+        s_senders[j] = s_peer[j];
+        s_begin[j] = 0;
+      } else if (q.mix_mode == kMixLossy) {
+        // only the last writer lands; slot j is this receiver's own
+        s_begin[j] = j;
+        if (last >= 0) {
+          const double ws = s_wh[last];
+          s_senders[j] = last;
+          s_alpha[j] = (float)(ws / (W + ws));
+          W = W + ws;
+          n_list = 1;
+        }
+      } else {
+        int k = below;
+        s_begin[j] = below;
+        for (int sdr = 0; sdr < K; ++sdr) {
+          if (s_peer[sdr] != j) continue;
+          const double ws = s_wh[sdr];
+          s_senders[k] = sdr;
+          s_alpha[k] = (float)(ws / (W + ws));               // one rounding to fp32
+          W = W + ws;                                        // w_j <- w_j + w_i
+          ++k;
+        }
+        n_list = cnt;
+      }
+      s_cnt[j] = n_list;
+      s_wnew[j] = W;
+      s_flags[j] = (unsigned char)((act ? kFlagActive : 0) | (cnt > 0 ? kFlagRecv : 0));
+    }
+    __syncthreads();   // schedule visible; every read of w / bpow by this CTA has returned
+    if (tid == 0) ticket = atomicAdd(q.ticket + layer, 1);
+  } else {
     const size_t row = (size_t)layer * K;
     for (int k = tid; k < K; k += THREADS) {
       s_senders[k] = SYM ? p.t.peer[row + k] : p.t.senders[row + k];
       s_alpha[k] = p.t.alpha[row + k];
       s_flags[k] = p.t.flags[row + k];
+      const int b = p.t.recv_off[(size_t)layer * (K + 1) + k];
+      s_begin[k] = b;
+      s_cnt[k] = p.t.recv_off[(size_t)layer * (K + 1) + k + 1] - b;
       if (HAS_V) {
         s_c1[k] = p.t.c1[row + k];
         s_c2[k] = p.t.c2[row + k];
       }
     }
-    for (int k = tid; k <= K; k += THREADS) s_recv_off[k] = p.t.recv_off[(size_t)layer * (K + 1) + k];
+    __syncthreads();   // schedule visible
   }
-  __syncthreads();   // schedule visible
 
   if (!p.all_active) {
     // straggler round: the flags decide which chunks are touched at all
@@ -173,7 +249,6 @@ __global__ void __launch_bounds__(THREADS, MINB)
   mbar_wait(bar, 0);
 
   // ---- phase 1: local step out of shared memory; y overwrites x in place, m' (v') -> HBM
-  const bool bulk_out = (p.hints & 4) != 0;     // outputs leave through TMA bulk stores instead of STG
   for (int idx = tid; idx < n_items; idx += THREADS) {
     const int i = idx >> log2C, c = idx & (C - 1);
     if (c >= ncols) continue;
@@ -182,26 +257,11 @@ __global__ void __launch_bounds__(THREADS, MINB)
     float4 v = HAS_V ? vs[idx] : float4{0.f, 0.f, 0.f, 0.f};
     const float4 y = local_step4<OPT>(xs[idx], gs[idx], m, v, p.s, HAS_V ? s_c1[i] : 0.f, HAS_V ? s_c2[i] : 0.f);
     const long long off = (long long)i * pad + (c << 2);
-    if (bulk_out) {
-      if (HAS_M) ms[idx] = m;
-      if (HAS_V) vs[idx] = v;
-    } else {
-      if (HAS_M) { if (p.hints & 2) st4_cs(mb + off, m); else st4(mb + off, m); }
-      if (HAS_V) { if (p.hints & 2) st4_cs(vb + off, v); else st4(vb + off, v); }
-    }
+    if (HAS_M) st4(mb + off, m);
+    if (HAS_V) st4(vb + off, v);
     xs[idx] = y;
   }
-  if (bulk_out && HAS_M) fence_proxy_async();
   __syncthreads();
-  if (bulk_out && HAS_M) {
-    // m' (v') of every active replica: one bulk store per (replica, array), spread like the loads
-    constexpr int NOUT = HAS_M ? NARR - 2 : 1;
-    for (int c = slot0; c < K * NOUT; c += THREADS) {
-      const int i = c / NOUT, a = 2 + (c - i * NOUT);
-      if (!(s_flags[i] & kFlagActive)) continue;
-      bulk_s2g((a == 2 ? mb : vb) + (long long)i * pad, xs + a * n_items + (i << log2C), chunk);
-    }
-  }
 
   if (SYM) {
     // ---- phase 2 (symmetric): every scalar column runs the K exchanges in worker order
@@ -220,37 +280,49 @@ __global__ void __launch_bounds__(THREADS, MINB)
       if (c >= ncols) continue;
       if (!s_flags[i]) continue;                                            // idle, no push received: 0 bytes
       float4 acc = xs[idx];
-      const int k_end = s_recv_off[i + 1];
-      for (int k = s_recv_off[i]; k < k_end; ++k) peer_update4(acc, xs[(s_senders[k] << log2C) + c], s_alpha[k]);
-      if (bulk_out) gs[idx] = acc;                                          // g is dead: its tile carries x out
-      else if (p.hints & 2) st4_cs(xb + (long long)i * pad + (c << 2), acc);
-      else st4(xb + (long long)i * pad + (c << 2), acc);
-    }
-    if (bulk_out) {
-      fence_proxy_async();
-      __syncthreads();
-      for (int i = slot0; i < K; i += THREADS)
-        if (s_flags[i]) bulk_s2g(xb + (long long)i * pad, gs + (i << log2C), chunk);
+      const int k0 = s_begin[i], k_end = k0 + s_cnt[i];
+      for (int k = k0; k < k_end; ++k) peer_update4(acc, xs[(s_senders[k] << log2C) + c], s_alpha[k]);
+      st4(xb + (long long)i * pad + (c << 2), acc);
     }
   }
-  if (bulk_out) bulk_commit_wait_read();   // shared memory must outlive the stores' reads
+
+  if (FUSED) {
+    // the CTA that drew the last ticket of its layer knows every other CTA has read the old
+    // state: it publishes the new push-sum weights / beta powers and re-arms the ticket
+    __shared__ int s_last;
+    const int tiles_in_layer = (int)(tab.prefix[lo + 1] - tab.prefix[lo]);
+    if (tid == 0) s_last = (ticket == tiles_in_layer - 1);
+    __syncthreads();
+    if (s_last) {
+      const SchedParams &q = p.sched;
+      const size_t row = (size_t)layer * K;
+      if (tid < K) {
+        if (!SYM) q.w[row + tid] = s_wnew[tid];
+        if (HAS_V) {
+          q.bpow[2 * (row + tid)] = s_bp[2 * tid];
+          q.bpow[2 * (row + tid) + 1] = s_bp[2 * tid + 1];
+        }
+      }
+      if (tid == 0) q.ticket[layer] = 0;
+    }
+  }
 }
 
 using TmaFn = void (*)(const UpdateParams, const PosTable);
 struct TmaVariant {
   int threads, minb;
-  TmaFn fn[3][2];   // [OPT][SYM]
+  TmaFn fn[3][2];       // [OPT][SYM]   schedule tables read from global memory (two launches)
+  TmaFn fused[3][2];    // [OPT][SYM]   schedule computed in the kernel (one launch); nullptr = not built
 };
-#define LAYUP_TMA_VARIANT(T, MB)                                                                              \
-  TmaVariant {                                                                                                \
-    T, MB, {                                                                                                  \
-      {layup_update_tma<OPT_SGD, false, T, MB>, layup_update_tma<OPT_SGD, true, T, MB>},                      \
-          {layup_update_tma<OPT_SGD_MOM, false, T, MB>, layup_update_tma<OPT_SGD_MOM, true, T, MB>},          \
-          {layup_update_tma<OPT_ADAMW, false, T, MB>, layup_update_tma<OPT_ADAMW, true, T, MB>},              \
-    }                                                                                                         \
-  }
+#define LAYUP_TMA_ROW(O, F, T, MB) {layup_update_tma<O, false, F, T, MB>, layup_update_tma<O, true, F, T, MB>}
+#define LAYUP_TMA_TABLE(F, T, MB) \
+  {LAYUP_TMA_ROW(OPT_SGD, F, T, MB), LAYUP_TMA_ROW(OPT_SGD_MOM, F, T, MB), LAYUP_TMA_ROW(OPT_ADAMW, F, T, MB)}
+#define LAYUP_TMA_NONE {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}}
 const TmaVariant kTma[] = {
-    LAYUP_TMA_VARIANT(256, 4), LAYUP_TMA_VARIANT(128, 8), LAYUP_TMA_VARIANT(512, 2), LAYUP_TMA_VARIANT(256, 2),
+    TmaVariant{256, 4, LAYUP_TMA_TABLE(false, 256, 4), LAYUP_TMA_TABLE(true, 256, 4)},
+    TmaVariant{128, 8, LAYUP_TMA_TABLE(false, 128, 8), LAYUP_TMA_NONE},
+    TmaVariant{512, 2, LAYUP_TMA_TABLE(false, 512, 2), LAYUP_TMA_NONE},
+    TmaVariant{256, 2, LAYUP_TMA_TABLE(false, 256, 2), LAYUP_TMA_NONE},
 };
 constexpr int kNumTma = sizeof(kTma) / sizeof(kTma[0]);
 
@@ -258,30 +330,40 @@ constexpr int kNumTma = sizeof(kTma) / sizeof(kTma[0]);
 
 int tma_num_variants() { return kNumTma; }
 
-size_t tma_smem_bytes(int K, int C, int opt) {
+size_t tma_smem_bytes(int K, int C, int opt, bool fused) {
   const int narr = opt == OPT_ADAMW ? 4 : opt == OPT_SGD_MOM ? 3 : 2;
-  return (size_t)K * C * sizeof(float4) * narr + 8 + sizeof(int) * (2 * (size_t)K + 1) +
-         sizeof(float) * K * (opt == OPT_ADAMW ? 3 : 1) + (size_t)K;
+  size_t b = (size_t)K * C * sizeof(float4) * narr + 8;                        // staged arrays + mbarrier
+  if (fused) b += sizeof(double) * K * (opt == OPT_ADAMW ? 4 : 2) + sizeof(int) * K;   // wh, wnew (, beta powers), peer
+  b += sizeof(int) * 3 * (size_t)K + sizeof(float) * K * (opt == OPT_ADAMW ? 3 : 1) + (size_t)K;
+  return b;
 }
+
+bool tma_has_fused(int variant) { return variant >= 0 && variant < kNumTma && kTma[variant].fused[0][0] != nullptr; }
 
 cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_bytes, int *threads, int *ctas_per_sm) {
   if (variant < 0 || variant >= kNumTma || opt < 0 || opt > 2) return cudaErrorInvalidValue;
   const TmaVariant &v = kTma[variant];
-  TmaFn f = v.fn[opt][symmetric ? 1 : 0];
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
-  int a = 0;
-  if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, f, v.threads, smem_bytes)) != cudaSuccess) return e;
+  int occ = 1 << 30;
+  for (TmaFn f : {v.fn[opt][symmetric ? 1 : 0], v.fused[opt][symmetric ? 1 : 0]}) {
+    if (!f) continue;
+    if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
+    int a = 0;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, f, v.threads, smem_bytes)) != cudaSuccess) return e;
+    occ = a < occ ? a : occ;
+  }
   *threads = v.threads;
-  *ctas_per_sm = a;
+  *ctas_per_sm = occ;
   return cudaSuccess;
 }
 
-cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, int grid, int smem_bytes,
-                              cudaStream_t s) {
+cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, int grid,
+                              int smem_bytes, cudaStream_t s) {
   const TmaVariant &v = kTma[variant];
-  v.fn[p.opt][p.symmetric ? 1 : 0]<<<grid, v.threads, smem_bytes, s>>>(p, tab);
+  TmaFn f = (fused ? v.fused : v.fn)[p.opt][p.symmetric ? 1 : 0];
+  if (!f) return cudaErrorInvalidValue;
+  f<<<grid, v.threads, smem_bytes, s>>>(p, tab);
   return cudaGetLastError();
 }
 

@@ -214,3 +214,33 @@ def test_argument_errors_of_the_new_fields():
     lu = LayUp(4, [100], 0.1, optimizer=OPT_ADAMW)
     assert lu.view(WHAT_V, 0).shape == (4, 100) and lu.view(WHAT_M, 0).shape == (4, 100)
     lu.close()
+
+
+@pytest.mark.parametrize("opt,mix,mu,skip", [(OPT_SGD, MIX_PUSHSUM, 0.0, 0.0), (OPT_SGD, MIX_PUSHSUM, 0.9, 0.25),
+                                             (OPT_SGD, MIX_LOSSY, 0.9, 0.1), (OPT_SGD, MIX_SYMMETRIC, 0.0, 0.25),
+                                             (OPT_ADAMW, MIX_PUSHSUM, 0.0, 0.25), (OPT_ADAMW, MIX_LOSSY, 0.0, 0.0),
+                                             (OPT_ADAMW, MIX_SYMMETRIC, 0.0, 0.0)])
+@pytest.mark.parametrize("K", [1, 2, 5, 16, 64])
+def test_single_launch_path_equals_two_launch_path(opt, mix, mu, skip, K, monkeypatch):
+    """Launch-latency-bound launches compute the schedule stage inside the update kernel (one
+    launch per round / per layer event); larger ones run the schedule kernel first.  Same bits,
+    same weights, and both equal the oracle."""
+    kw = ADAM if opt == OPT_ADAMW else {}
+    outs, launches = [], []
+    for fused in ("1", "0"):
+        monkeypatch.setenv("LAYUP_FUSED", fused)
+        w, lu, ref, _ = _pair(K, NUMEL, 1e-3, mu, 31, skip, opt, mix, **kw)
+        n0 = lu.layup_launch_count()
+        _run(w, lu, ref, None, 4)
+        # per-layer events take the same path
+        for l in range(w.L):
+            synth.fill_grad_(w, 4, l, lu.view(WHAT_G, l))
+        for l in reversed(range(w.L)):
+            lu.layup_layer_update(4, l)
+        lu.layup_sync()
+        launches.append(lu.layup_launch_count() - n0)
+        outs.append([lu.view(WHAT_X, l).cpu().numpy().copy() for l in range(w.L)] + [lu.layup_weights()])
+        lu.close()
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+    assert launches[0] == 4 + len(NUMEL) and launches[1] == 2 * launches[0]
