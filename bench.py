@@ -91,15 +91,15 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def committed_traffic(name):
+def committed_traffic(name, optimizer="sgd"):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture
-    (profiles/traffic.csv, see profiles/traffic.md); None if this workload was not captured."""
+    (profiles/traffic.csv, see profiles/traffic.md); None if this (workload, optimizer) was not captured."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(p):
         import csv
         with open(p) as f:
             for row in csv.DictReader(f):
-                if row["workload"] == name:
+                if row["workload"] == name and row["optimizer"] == optimizer:
                     return float(row["dram_bytes_per_launch"])
     return None
 
@@ -310,7 +310,7 @@ def run_ours(args, w, rank, world, local_rank):
     bytes_per_launch = sum(bts) / max(n_k, 1)
     achieved = bytes_per_launch / (k_avg_ms * 1e-3) / 1e9 if k_avg_ms > 0 else 0.0
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": committed_traffic(w.name) if (args.optimizer, args.mix) == ("sgd", "pushsum") else None, "kernel": "layup_update_kernel",
+                "traffic": committed_traffic(w.name, args.optimizer) if args.mix == "pushsum" else None, "kernel": "layup_update_tma",
                 "kernel_ms_avg": k_avg_ms, "kernel_launches": n_k, "algorithmic_bytes_per_launch": bytes_per_launch,
                 "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0}
 

@@ -158,13 +158,15 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   ctx->section = section_floats(cfg);
 
   // tile shape: C float4 columns per replica (power of two, >= 8), K*C items per tile.
-  // ~1024 items (48 KB staged with momentum, 4 CTAs/SM) measured best on B200; chunks are
-  // kept >= 512 B per replica when the staging still fits comfortably (large K, no momentum).
+  // Measured on B200: ~1024 items per CTA (48 KB staged with momentum, 4 CTAs/SM) is
+  // best while a replica's row of the tile is >= 1 KB; for K >= 32 rows of 1 KB (C = 64) beat more
+  // CTAs per SM as long as two CTAs still fit (staged bytes <= 112 KB).
   const int items_env = env_int("LAYUP_TILE_ITEMS", 0);
   const int items_target = std::max(256, items_env > 0 ? items_env : 1024);
   int C = 8;
   while ((long long)cfg->K * C * 2 <= items_target && C < 4096) C *= 2;
-  if (items_env <= 0 && ctx->n_sections == 2 && C < 32 && cfg->K <= 64) C = 32;
+  if (items_env <= 0)
+    while (C < 64 && (long long)cfg->K * (2 * C) * 16 * ctx->n_sections <= 112 * 1024) C *= 2;
   if (items_env <= 0) {
     // a whole round of fewer work items than ~4 per SM is latency bound: smaller tiles, more CTAs
     // (B200: 148 SMs; chunks stay >= 256 B per replica)
@@ -260,7 +262,11 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   CU_TRY_INIT(cudaMemset(ctx->d_ticket, 0, sizeof(int32_t) * L));
   CU_TRY_INIT(cudaMalloc(&ctx->d_active_scratch, (size_t)K));
   CU_TRY_INIT(cudaMalloc(&ctx->d_dist, sizeof(double) * L * K));
-  if (ctx->engine == 1 && env_int("LAYUP_TMA2D", 1) != 0 && K <= 256 && C * 4 <= 256) {
+  // 2-D tile loads replace K*arrays 1-D bulk copies per CTA by one per array.  Measured on B200: a
+  // clear win without momentum (K = 16: 6.27 -> 6.94 TB/s) and from 64 copies per CTA up; at
+  // K = 16 with momentum (48 copies) the 1-D form is 0.2 % ahead, so it is kept there.
+  const bool want_2d = env_int("LAYUP_TMA2D", (ctx->n_sections == 2 || K * ctx->n_sections >= 64) ? 1 : 0) != 0;
+  if (ctx->engine == 1 && want_2d && K <= 256 && C * 4 <= 256) {
     // One tensor map per (section, layer): rank 2, inner dim = the padded slice, outer dim = the K
     // replicas (stride = pad), box = [K][C*4 floats], no swizzle, zero fill past the slice end.
     typedef CUresult (*EncodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,

@@ -244,3 +244,34 @@ def test_single_launch_path_equals_two_launch_path(opt, mix, mu, skip, K, monkey
     for a, b in zip(*outs):
         assert np.array_equal(a, b)
     assert launches[0] == 4 + len(NUMEL) and launches[1] == 2 * launches[0]
+
+
+@pytest.mark.parametrize("opt,mix", [(OPT_SGD, MIX_PUSHSUM), (OPT_ADAMW, MIX_PUSHSUM), (OPT_ADAMW, MIX_SYMMETRIC)])
+def test_pads_stay_zero_and_nothing_is_written_out_of_bounds(opt, mix):
+    """Bounds check of our own (compute-sanitizer is closed on this pool): every slice is padded to
+    32 floats; the kernels process the padded length and must leave every pad float of every
+    section exactly zero, for ragged sizes on both sides of a tile boundary."""
+    K = 8
+    numel = [1, 31, 33, 127, 129, 255 * 4 + 1, 4096 + 3, 8191, 1000]
+    kw = ADAM if opt == OPT_ADAMW else {}
+    lu = LayUp(K, numel, 1e-3, 0.9 if opt == OPT_SGD else 0.0, 2, 0, 0.25, optimizer=opt, mix_mode=mix, **kw)
+    n_sec = 4 if opt == OPT_ADAMW else 3
+    for step in range(6):
+        for l in range(len(numel)):
+            lu.view(WHAT_X if step == 0 else WHAT_G, l).normal_(0, 1)
+            lu.view(WHAT_G, l).normal_(0, 1)
+        if step % 2:
+            lu.layup_round(step)
+        else:
+            for l in reversed(range(len(numel))):
+                lu.layup_layer_update(step, l)
+        lu.layup_sync()
+    for what in range(n_sec):
+        for l, n in enumerate(numel):
+            pad = (n + 31) // 32 * 32
+            p0, _ = lu.ptr(what, 0, l)
+            off = (p0 - lu._base) // 4
+            full = lu._arena_f32.as_strided((K, pad), (pad, 1), off)
+            assert bool((full[:, n:] == 0).all()), (what, l)
+            assert bool(torch.isfinite(full).all())
+    lu.close()
