@@ -147,6 +147,14 @@ int layup_schedule(layup_ctx *ctx, int64_t step, int32_t *peer /*[L*K]*/, uint8_
 /* Current push-sum weights w[l*K+i], after all work issued so far. */
 int layup_weights(layup_ctx *ctx, double *w /*[L*K]*/);
 
+/* Checkpoint / resume.  Everything the library owns besides the caller's arena: the push-sum
+ * weights w[L*K], AdamW's running beta powers bpow[L*K*2] = (beta1^t, beta2^t)
+ * per (layer, replica) (NULL unless the optimizer is AdamW) and the step each layer expects
+ * next, next_step[L].  HOST arrays.  A ctx created with the same config over a copy of the
+ * arena and given these three continues bit-identically.  Synchronous. */
+int layup_state_export(layup_ctx *ctx, double *w, double *bpow, int64_t *next_step);
+int layup_state_import(layup_ctx *ctx, const double *w, const double *bpow, const int64_t *next_step);
+
 /* Model disagreement (PAPER.md:389-395 Fig. A1; eq. (9)): for every layer l and
  * replica i, dist[l*K+i] = sum_e (x_i[e] - xbar[e])^2, where xbar = (1/K) sum_i x_i (weighted == 0,
  * the paper's plain average) or xbar = sum_i w_i x_i with the current push-sum weights

@@ -38,7 +38,7 @@ class _Config(ctypes.Structure):
 
 EXPORTS = ["layup_arena_bytes", "layup_init", "layup_destroy", "layup_ptr", "layup_set_lr",
            "layup_layer_update", "layup_round", "layup_round_host", "layup_sync", "layup_peer",
-           "layup_schedule", "layup_weights", "layup_disagreement", "layup_profile", "layup_profile_read", "layup_launch_count",
+           "layup_schedule", "layup_weights", "layup_state_export", "layup_state_import", "layup_disagreement", "layup_profile", "layup_profile_read", "layup_launch_count",
            "layup_last_error"]
 
 
@@ -65,6 +65,8 @@ def load_library():
         "layup_peer": [c.c_uint64, i64, i32, i32, i32, c.POINTER(i32)],
         "layup_schedule": [vp, i64, vp, vp],
         "layup_weights": [vp, vp],
+        "layup_state_export": [vp, vp, vp, vp],
+        "layup_state_import": [vp, vp, vp, vp],
         "layup_disagreement": [vp, i32, vp],
         "layup_profile": [vp, i32],
         "layup_profile_read": [vp, c.POINTER(i64), c.POINTER(c.c_double)],
@@ -193,6 +195,23 @@ class LayUp:
         w = np.empty((self.L, self.K), dtype=np.float64)
         _check(self.lib.layup_weights(self.ctx, w.ctypes.data), self.ctx)
         return w
+
+    def layup_state_export(self):
+        """-> (w [L,K] fp64, bpow [L,K,2] fp64 or None, next_step [L] int64)."""
+        w = np.empty((self.L, self.K), dtype=np.float64)
+        bp = np.empty((self.L, self.K, 2), dtype=np.float64) if self.optimizer == OPT_ADAMW else None
+        ns = np.empty(self.L, dtype=np.int64)
+        _check(self.lib.layup_state_export(self.ctx, w.ctypes.data, bp.ctypes.data if bp is not None else None,
+                                           ns.ctypes.data), self.ctx)
+        return w, bp, ns
+
+    def layup_state_import(self, w, bpow, next_step):
+        w = np.ascontiguousarray(w, dtype=np.float64)
+        ns = np.ascontiguousarray(next_step, dtype=np.int64)
+        bp = np.ascontiguousarray(bpow, dtype=np.float64) if bpow is not None else None
+        assert w.shape == (self.L, self.K) and ns.shape == (self.L,)
+        _check(self.lib.layup_state_import(self.ctx, w.ctypes.data, bp.ctypes.data if bp is not None else None,
+                                           ns.ctypes.data), self.ctx)
 
     def layup_disagreement(self, weighted: bool = False) -> np.ndarray:
         d = np.empty((self.L, self.K), dtype=np.float64)

@@ -524,6 +524,32 @@ extern "C" int layup_weights(layup_ctx *ctx, double *w) {
   return LAYUP_OK;
 }
 
+extern "C" int layup_state_export(layup_ctx *ctx, double *w, double *bpow, int64_t *next_step) {
+  if (!ctx || !w || !next_step) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  if (ctx->opt == OPT_ADAMW && !bpow) return fail(ctx, LAYUP_EINVAL, "bpow is NULL but the optimizer is AdamW");
+  int rc = layup_sync(ctx);
+  if (rc) return rc;
+  const size_t n = (size_t)ctx->L * ctx->K;
+  CU_TRY(ctx, cudaMemcpy(w, ctx->d_w, sizeof(double) * n, cudaMemcpyDeviceToHost));
+  if (ctx->opt == OPT_ADAMW) CU_TRY(ctx, cudaMemcpy(bpow, ctx->d_bpow, sizeof(double) * 2 * n, cudaMemcpyDeviceToHost));
+  for (int l = 0; l < ctx->L; ++l) next_step[l] = ctx->next_step[l];
+  return LAYUP_OK;
+}
+
+extern "C" int layup_state_import(layup_ctx *ctx, const double *w, const double *bpow, const int64_t *next_step) {
+  if (!ctx || !w || !next_step) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  if (ctx->opt == OPT_ADAMW && !bpow) return fail(ctx, LAYUP_EINVAL, "bpow is NULL but the optimizer is AdamW");
+  for (int l = 0; l < ctx->L; ++l)
+    if (next_step[l] < 0 || next_step[l] > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "next_step[%d] outside [0, 2^32)", l);
+  int rc = layup_sync(ctx);
+  if (rc) return rc;
+  const size_t n = (size_t)ctx->L * ctx->K;
+  CU_TRY(ctx, cudaMemcpy(ctx->d_w, w, sizeof(double) * n, cudaMemcpyHostToDevice));
+  if (ctx->opt == OPT_ADAMW) CU_TRY(ctx, cudaMemcpy(ctx->d_bpow, bpow, sizeof(double) * 2 * n, cudaMemcpyHostToDevice));
+  for (int l = 0; l < ctx->L; ++l) ctx->next_step[l] = next_step[l];
+  return LAYUP_OK;
+}
+
 extern "C" int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist) {
   if (!ctx || !dist) return fail(ctx, LAYUP_EINVAL, "NULL argument");
   int rc = layup_sync(ctx);

@@ -275,3 +275,41 @@ def test_pads_stay_zero_and_nothing_is_written_out_of_bounds(opt, mix):
             assert bool((full[:, n:] == 0).all()), (what, l)
             assert bool(torch.isfinite(full).all())
     lu.close()
+
+
+@pytest.mark.parametrize("opt", [OPT_SGD, OPT_ADAMW])
+def test_checkpoint_resume_is_bit_identical(opt):
+    """layup_state_export / layup_state_import + a copy of the arena = a resumable snapshot."""
+    K = 8
+    kw = ADAM if opt == OPT_ADAMW else {}
+    mu = 0.9 if opt == OPT_SGD else 0.0
+    w, a, _, _ = _pair(K, NUMEL, 1e-3, mu, 17, 0.25, opt, MIX_PUSHSUM, **kw)
+    def grads(lu, step):
+        for l in range(w.L):
+            synth.fill_grad_(w, step, l, lu.view(WHAT_G, l))
+
+    for step in range(4):
+        grads(a, step)
+        a.layup_round(step)
+    # a layer-wise partial round: the three last layers are one step ahead at the snapshot
+    grads(a, 4)
+    for l in (w.L - 1, w.L - 2, w.L - 3):
+        a.layup_layer_update(4, l)
+    state = a.layup_state_export()
+    b = LayUp(K, NUMEL, 1e-3, mu, 17, 0, 0.25, optimizer=opt, mix_mode=MIX_PUSHSUM, **kw)
+    b._arena_f32.copy_(a._arena_f32)
+    b.layup_state_import(*state)
+    with pytest.raises(LayUpError):
+        b.layup_round(4)                              # layers disagree about the step: refused
+    for lu in (a, b):
+        for l in reversed(range(w.L - 3)):
+            lu.layup_layer_update(4, l)
+        for step in range(5, 8):
+            grads(lu, step)
+            lu.layup_round(step)
+        lu.layup_sync()
+    for what in ([WHAT_X, WHAT_M] + ([WHAT_V] if opt == OPT_ADAMW else [])):
+        for l in range(w.L):
+            assert torch.equal(a.view(what, l), b.view(what, l)), (what, l)
+    assert np.array_equal(a.layup_weights(), b.layup_weights())
+    a.close(); b.close()
