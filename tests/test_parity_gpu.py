@@ -290,3 +290,60 @@ def test_full_size_sampled_parity(name, rounds):
     lu.close()
     del lu
     torch.cuda.empty_cache()
+
+
+def test_maximum_replica_count():
+    """K = LAYUP_MAX_K = 1024 replicas (the LDG kernels take over when the tile of all K replicas no
+    longer fits the TMA staging): schedule, weights and parameters against the oracle."""
+    K, numel = 1024, [700, 33, 2049]
+    w = synth.Workload("kmax", K, tuple(numel), 0.01, 0.9, 3, 77, grad_std=1e-2, skip_prob=0.1)
+    lu, ref, _ = make_pair(w)
+    for step in range(3):
+        grads = load_grads(w, lu, step)
+        peer, active = lu.layup_schedule(step)
+        rp, ra = oracle.schedule(w.seed, step, w.L, w.K, w.peer_mode, w.skip_prob)
+        assert np.array_equal(peer, rp) and np.array_equal(active, ra)
+        lu.layup_round(step)
+        lu.layup_sync()
+        ref.round(step, grads)
+        _, u = compare(w, lu, ref, REL_TOL_ROUND, "K=1024 step %d" % step)
+        assert u == 0
+        assert np.array_equal(lu.layup_weights(), ref.w)
+    lu.close()
+    with pytest.raises(LayUpError) as e:
+        LayUp(1025, [10], 0.1)
+    assert e.value.code == LAYUP_EINVAL
+
+
+def test_layer_larger_than_2_to_31_elements():
+    """64-bit indexing: one layer of 2^31 + 1000 elements per replica (8.6 GB), K = 2, sampled
+    columns around the start, the 2^31 boundary and the ragged tail against the oracle."""
+    n = (1 << 31) + 1000
+    free, _ = torch.cuda.mem_get_info()
+    if 2 * 2 * (n + 32) * 4 + (6 << 30) > free:
+        pytest.skip("needs 35 GB of HBM")
+    K = 2
+    lu = LayUp(K, [n, 100], 0.5, 0.0, 5)
+    cols = torch.cat([torch.arange(0, 300), torch.arange((1 << 31) - 300, (1 << 31) + 300), torch.arange(n - 300, n),
+                      torch.arange(3 * (1 << 29) - 50, 3 * (1 << 29) + 50)]).cuda()
+    ref = oracle.Oracle([int(cols.numel()), 100], K, 0.5, 0.0, 5)
+    x = lu.view(WHAT_X, 0)
+    for i in range(K):                                   # cheap deterministic fill of 8.6 GB per replica
+        x[i].copy_(torch.arange(n, device="cuda", dtype=torch.float32).mul_(1e-9 * (i + 1)))
+    lu.view(WHAT_X, 1).normal_(0, 1)
+    ref.x[0][:] = x[:, cols].cpu().numpy()
+    ref.x[1][:] = lu.view(WHAT_X, 1).cpu().numpy()
+    for step in range(2):
+        g = lu.view(WHAT_G, 0)
+        for i in range(K):
+            g[i].copy_(torch.arange(n, device="cuda", dtype=torch.float32).mul_(1e-10 * (step + 1) * (i + 2)))
+        lu.view(WHAT_G, 1).normal_(0, 1)
+        grads = [g[:, cols].cpu().numpy(), lu.view(WHAT_G, 1).cpu().numpy()]
+        lu.layup_round(step)
+        lu.layup_sync()
+        ref.round(step, grads)
+        assert max_ulp(x[:, cols].cpu().numpy(), ref.x[0]) == 0
+        assert max_ulp(lu.view(WHAT_X, 1).cpu().numpy(), ref.x[1]) == 0
+    lu.close()
+    del lu, x, g
+    torch.cuda.empty_cache()
