@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- param-updates/s and effective HBM GB/s of the LayUp update+gossip round.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME|all] [--impl ours|reference]
+                  [--optimizer sgd|adamw] [--mix pushsum|lossy|symmetric] [--mode round|layers]
 
 A "step" is one layup_round(): the whole hot path (straggler mask, peer choice, push-sum
 weights, local step, push, peer mix, reverse-layer work list) over all K replicas of all
@@ -246,7 +247,8 @@ def run_ours(args, w, rank, world, local_rank):
     dist = None
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if not dist.is_initialized():
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     def barrier():
         if dist is not None:
@@ -374,11 +376,16 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    w = get_workload(args.config)
-    if args.impl == "reference":
-        run_reference(args, w, rank, world)
-    else:
-        run_ours(args, w, rank, world, local_rank)
+    # --config all: the per-config report north_star asks for, one JSON line per BASELINE config
+    # (the default invocation prints exactly one line, for configs[2])
+    names = [w.name for w in synth.workloads()] if args.config == "all" else [args.config]
+    for name in names:
+        w = get_workload(name)
+        if args.impl == "reference":
+            run_reference(args, w, rank, world)
+        else:
+            run_ours(args, w, rank, world, local_rank)
+            torch.cuda.empty_cache()
 
 
 if __name__ == "__main__":

@@ -1,14 +1,19 @@
-// TMA-staged form of the fused local-step + gossip-mix kernel (see update.cu for the rule).
+// TMA-staged form of the fused local-step + gossip-mix kernel (rule.cuh holds the arithmetic).
 //
-// Same work item -- (layer, tile of C float4 columns) for ALL K replicas, one CTA per item --
-// but the K x {x, g, m} chunks of the tile are brought into shared memory by 1-D bulk
-// copies (cp.async.bulk, the TMA engine; SASS UBLKCP) completing on one mbarrier, so the
-// whole tile (K*C*16 B * 3) is in flight per CTA without holding registers.  The local step
-// then runs out of shared memory, y overwrites x in place (the "send" is an on-chip read,
-// PAPER.md:101), m' (and AdamW's v') go straight to HBM, and after one CTA barrier every
-// receiver folds its senders and writes x once.  HBM traffic is unchanged: 12 B (SGD) / 20 B
-// (momentum) / 28 B (AdamW) per parameter update.  Template parameters: OPT = local optimiser
-// (rule.cuh), SYM = symmetric pairwise averaging instead of the push-sum fold.
+// Work item = (layer, tile of C float4 columns) for ALL K replicas, one CTA per item.  The tile
+// of every array (x, g, m, v) is brought into shared memory by the TMA engine, completing on one
+// mbarrier, so the whole tile (K*C*16 B per array) is in flight per CTA without holding registers:
+//   - when every replica is active and the box fits the TMA limits: ONE 2-D tiled copy per array
+//     (cp.async.bulk.tensor.2d, SASS UTMALDG.2D) through a tensor map that views a layer section
+//     as [K rows][padded slice];
+//   - otherwise K x arrays 1-D bulk copies (cp.async.bulk, SASS UBLKCP), spread over all warps,
+//     skipping what an idle replica does not need.
+// The local step then runs out of shared memory, y overwrites x in place (the "send" is an
+// on-chip read), m' (and AdamW's v') go straight to HBM, and after one CTA barrier
+// every receiver folds its senders and writes x once.  HBM traffic: 12 B (SGD) / 20 B (momentum) /
+// 28 B (AdamW) per parameter update, nothing read or written twice.
+// Template parameters: OPT = local optimiser (rule.cuh), SYM = symmetric pairwise averaging
+// instead of the push-sum fold, FUSED = the schedule stage runs in this kernel (one launch).
 #include "layup_internal.cuh"
 #include "philox.cuh"
 #include "rule.cuh"
