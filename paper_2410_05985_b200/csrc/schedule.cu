@@ -24,7 +24,6 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
   double *s_wh = reinterpret_cast<double *>(sm);                 // [K]
   int *s_peer = reinterpret_cast<int *>(s_wh + K);               // [K]
   int *s_cnt = s_peer + K;                                       // [K]
-  int *s_off = s_cnt + K;                                        // [K+1]
 
   const int layer = p.layer_begin + blockIdx.x;
   const int i = threadIdx.x;
@@ -53,27 +52,31 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
   }
   __syncthreads();
 
-  int cnt = 0;
+  // CSR by receiver without a serial prefix sum: the senders of receivers below i are exactly the
+  // pushes whose peer index is below i; one pass over the K peers gives count, offset and last writer
+  int cnt = 0, off = 0, last = -1;
   if (i < K) {
-    for (int s = 0; s < K; ++s) cnt += (s_peer[s] == i);
-    // entries of the sender list: all pushes, the last writer only, or none (symmetric)
-    s_cnt[i] = p.mix_mode == kMixPushSum ? cnt : p.mix_mode == kMixLossy ? (cnt > 0 ? 1 : 0) : 0;
+    for (int s = 0; s < K; ++s) {
+      const int pr = s_peer[s];
+      cnt += (pr == i);
+      off += (pr >= 0 && pr < i);
+      if (pr == i) last = s;
+    }
   }
-  __syncthreads();
-  if (i == 0) {
-    int run = 0;
-    for (int j = 0; j < K; ++j) { s_off[j] = run; run += s_cnt[j]; }
-    s_off[K] = run;
+  // entries of the sender list: all pushes, the last writer only, or none (symmetric)
+  const int n_list = p.mix_mode == kMixPushSum ? cnt : p.mix_mode == kMixLossy ? (cnt > 0 ? 1 : 0) : 0;
+  if (p.mix_mode != kMixPushSum) {
+    // shortened lists: offset = entries of the receivers below i
+    if (i < K) s_cnt[i] = n_list;
+    __syncthreads();
+    off = 0;
+    if (i < K)
+      for (int r = 0; r < i; ++r) off += s_cnt[r];
   }
-  __syncthreads();
 
   if (i < K) {
     double W = s_wh[i];
-    int k = s_off[i];
-    int last = -1;
-    if (p.mix_mode == kMixLossy)
-      for (int s = 0; s < K; ++s)
-        if (s_peer[s] == i) last = s;
+    int k = off;
     for (int s = 0; s < K && p.mix_mode != kMixSymmetric; ++s) {
       if (s_peer[s] != i) continue;
       if (p.mix_mode == kMixLossy && s != last) continue;        // overwritten: skipped
@@ -85,8 +88,8 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
     }
     if (p.mix_mode != kMixSymmetric) p.w[row + i] = W;
     p.t.flags[row + i] = (unsigned char)((act ? kFlagActive : 0) | (cnt > 0 ? kFlagRecv : 0));
-    p.t.recv_off[(size_t)layer * (K + 1) + i] = s_off[i];
-    if (i == 0) p.t.recv_off[(size_t)layer * (K + 1) + K] = s_off[K];
+    p.t.recv_off[(size_t)layer * (K + 1) + i] = off;
+    if (i == K - 1) p.t.recv_off[(size_t)layer * (K + 1) + K] = off + n_list;
   }
 }
 
@@ -104,7 +107,7 @@ __global__ void layup_peers_only_kernel(uint64_t seed, uint32_t step, uint32_t s
 
 cudaError_t launch_schedule(const SchedParams &p, int n_layers, cudaStream_t s) {
   const int threads = ((p.K + 31) / 32) * 32;
-  const size_t smem = sizeof(double) * p.K + sizeof(int) * (3 * (size_t)p.K + 1);
+  const size_t smem = sizeof(double) * p.K + sizeof(int) * 2 * (size_t)p.K;
   layup_schedule_kernel<<<n_layers, threads, smem, s>>>(p);
   return cudaGetLastError();
 }
