@@ -51,6 +51,8 @@ def parse():
                     help="local step: the config's SGD(+momentum) [default, BASELINE.json] or AdamW (NEXT-3)")
     ap.add_argument("--mix", default="pushsum", choices=["pushsum", "lossy", "symmetric"],
                     help="mixer: push-sum fold [default, BASELINE.json], contention-lossy or symmetric (NEXT-4)")
+    ap.add_argument("--skip-prob", type=float, default=None,
+                    help="override the workload's straggler probability (configs[3] semantics on any shape)")
     ap.add_argument("--mode", default="round", choices=["round", "layers"],
                     help="round: one persistent launch per step; layers: L per-layer launches on 4 streams")
     return ap.parse_args()
@@ -381,6 +383,8 @@ def main():
     names = [w.name for w in synth.workloads()] if args.config == "all" else [args.config]
     for name in names:
         w = get_workload(name)
+        if args.skip_prob is not None:
+            w = synth.shrink(w, w.numel, skip_prob=args.skip_prob)
         if args.impl == "reference":
             run_reference(args, w, rank, world)
         else:
