@@ -390,6 +390,10 @@ def main():
         else:
             run_ours(args, w, rank, world, local_rank)
             torch.cuda.empty_cache()
+    if world > 1 and args.impl != "reference":
+        import torch.distributed as dist
+        if dist.is_initialized():
+            dist.destroy_process_group()
 
 
 if __name__ == "__main__":
