@@ -95,3 +95,14 @@ def test_product_does_not_import_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_2410_05985_b200\b", src, flags=re.M), f
             assert "#include \"../paper" not in src
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/layup.h is a C boundary: it compiles as C99 with no C++ or torch types in it."""
+    import subprocess
+    src = tmp_path / "use_layup.c"
+    src.write_text('#include "layup.h"\n'
+                   'int probe(void) { layup_config c; size_t n = 0; c.K = 1; c.L = 0; c.numel = 0;\n'
+                   '  return layup_arena_bytes(&c, &n) == LAYUP_EINVAL ? (int)sizeof(c) : -1; }\n')
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"),
+                           "-c", str(src), "-o", str(tmp_path / "use_layup.o")])
