@@ -162,9 +162,10 @@ int layup_state_import(layup_ctx *ctx, const double *w, const double *bpow, cons
  * parameter) after all work issued so far; dist is a HOST array.  Synchronous. */
 int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist /*[L*K]*/);
 
-/* Device time of the fused update kernel, measured with CUDA events on the launch
- * stream: enable, run, layup_sync(), read (and reset).  launches = update-kernel
- * launches timed, total_ms = sum of their durations. */
+/* Device time of the path's kernels, measured with CUDA events on the launch stream around
+ * every launching call's kernels (the schedule kernel, a few microseconds, and the fused update
+ * kernel): enable, run, layup_sync(), read (and reset).  launches = launching calls timed,
+ * total_ms = sum of their durations. */
 int layup_profile(layup_ctx *ctx, int32_t enable);
 int layup_profile_read(layup_ctx *ctx, int64_t *launches, double *total_ms);
 

@@ -43,6 +43,7 @@ struct layup_ctx {
   SchedTables t{};
   int32_t *d_peer_scratch = nullptr, *d_ticket = nullptr;
   void *d_tmaps = nullptr;                // [n_sections][L] CUtensorMap: 2-D tiled view [K][pad] of every layer section
+  bool pdl = true;                        // programmatic dependent launch of the update kernel behind the schedule kernel
   bool fused_ok = false;                  // the single-launch path exists for this ctx (K, engine, variant)
   long long fused_max_tiles = 0;          // ... and is taken by launches of at most this many work items
   unsigned char *d_active_scratch = nullptr;
@@ -216,6 +217,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   ctx->engine = env_int("LAYUP_ENGINE", 1);
   ctx->variant = env_int("LAYUP_VARIANT", 0);
   ctx->launch_shape = env_int("LAYUP_PERSISTENT", -1);
+  ctx->pdl = env_int("LAYUP_PDL", 1) != 0;
   if (ctx->engine == 1) {
     // TMA-staged kernel stages x, g (, m) of the whole tile: fall back to the LDG kernel if it does not fit
     if (ctx->variant < 0 || ctx->variant >= tma_num_variants()) ctx->variant = 0;
@@ -234,6 +236,8 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   // launches of up to this many work items are launch-latency bound: one fused launch beats two
   // (measured on B200 with every launch fused: K = 8 ties, K = 16 loses 8 %, K = 64 loses 45 % on
   //  HBM-sized rounds -- the redundant schedule stage is only free while the launch is latency bound)
+  //  (K = 8 always fused: per-layer events 3.03 -> 2.97 ms per round, but AdamW rounds -0.7 % and
+  //  straggler rounds -12 %, where the schedule stage sits in front of the loads: not done.)
   const int waves = env_int("LAYUP_FUSED_WAVES", 4);
   ctx->fused_max_tiles = (long long)waves * ctx->n_sm * ctx->ctas_per_sm;
   const int cap = env_int("LAYUP_CTAS_PER_SM", 0);
@@ -355,6 +359,14 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   sp.lr = (double)ctx->lr; sp.beta1 = (double)ctx->beta1; sp.beta2 = (double)ctx->beta2;
   sp.ticket = ctx->d_ticket;
   const bool fused = ctx->fused_ok && ctx->tile_prefix[pos_end] - ctx->tile_prefix[pos_begin] <= ctx->fused_max_tiles;
+  // profiling brackets the whole issue: the schedule kernel (a few us, overlapped with the update
+  // kernel's prologue by the programmatic dependent launch) and the update kernel(s)
+  std::pair<cudaEvent_t, cudaEvent_t> ev{nullptr, nullptr};
+  if (ctx->profiling) {
+    if (!ctx->prof_pool.empty()) { ev = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
+    else { CU_TRY(ctx, cudaEventCreate(&ev.first)); CU_TRY(ctx, cudaEventCreate(&ev.second)); }
+    CU_TRY(ctx, cudaEventRecord(ev.first, s));
+  }
   if (!fused) CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
 
   UpdateParams up{};
@@ -376,12 +388,6 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   const long long tiles = up.tile_end - up.tile_begin;
   const long long resident = (long long)ctx->n_sm * ctx->ctas_per_sm;
 
-  std::pair<cudaEvent_t, cudaEvent_t> ev{nullptr, nullptr};
-  if (ctx->profiling) {
-    if (!ctx->prof_pool.empty()) { ev = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
-    else { CU_TRY(ctx, cudaEventCreate(&ev.first)); CU_TRY(ctx, cudaEventCreate(&ev.second)); }
-    CU_TRY(ctx, cudaEventRecord(ev.first, s));
-  }
   int n_launch = 0;
   if (ctx->engine == 1) {
     // grouped launch(es): one CTA per work item; the work-list table travels in the kernel parameters
@@ -398,7 +404,8 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
       if (n == 0) return fail(ctx, LAYUP_EINVAL, "layer %d has more than 2^31 tiles", L - 1 - q0);
       tab.prefix[n] = ctx->tile_prefix[q0 + n] - t0;
       tab.n = n;
-      CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, fused, (int)tab.prefix[n], ctx->smem, s));
+      // only the first update launch directly follows the schedule kernel on the stream
+      CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, fused, ctx->pdl && n_launch == 0, (int)tab.prefix[n], ctx->smem, s));
       q0 += n;
       ++n_launch;
     }

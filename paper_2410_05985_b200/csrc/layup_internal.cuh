@@ -102,7 +102,7 @@ int tma_num_variants();
 size_t tma_smem_bytes(int K, int C, int opt, bool fused);
 bool tma_has_fused(int variant);
 cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_bytes, int *threads, int *ctas_per_sm);
-cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, int grid,
+cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, bool pdl, int grid,
                               int smem_bytes, cudaStream_t s);
 
 }  // namespace layup

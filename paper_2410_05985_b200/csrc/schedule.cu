@@ -25,6 +25,9 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
   int *s_peer = reinterpret_cast<int *>(s_wh + K);               // [K]
   int *s_cnt = s_peer + K;                                       // [K]
 
+  // the update kernel behind this one on the stream may start now (it waits for this grid's
+  // completion with griddepcontrol.wait before it reads the tables)
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int layer = p.layer_begin + blockIdx.x;
   const int i = threadIdx.x;
   const size_t row = (size_t)layer * K;

@@ -220,6 +220,9 @@ __global__ void __launch_bounds__(THREADS, MINB)
     __syncthreads();   // schedule visible; every read of w / bpow by this CTA has returned
     if (tid == 0) ticket = atomicAdd(q.ticket + layer, 1);
   } else {
+    // Programmatic dependent launch: this kernel may start while the schedule kernel in front of it
+    // on the stream is still running (its tile loads above do not depend on it); the tables do.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const size_t row = (size_t)layer * K;
     for (int k = tid; k < K; k += THREADS) {
       s_senders[k] = SYM ? p.t.peer[row + k] : p.t.senders[row + k];
@@ -363,13 +366,28 @@ cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_byte
   return cudaSuccess;
 }
 
-cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, int grid,
+cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, bool pdl, int grid,
                               int smem_bytes, cudaStream_t s) {
   const TmaVariant &v = kTma[variant];
   TmaFn f = (fused ? v.fused : v.fn)[p.opt][p.symmetric ? 1 : 0];
   if (!f) return cudaErrorInvalidValue;
-  f<<<grid, v.threads, smem_bytes, s>>>(p, tab);
-  return cudaGetLastError();
+  if (fused) {
+    f<<<grid, v.threads, smem_bytes, s>>>(p, tab);
+    return cudaGetLastError();
+  }
+  // after the schedule kernel on the same stream: programmatic stream serialization lets this
+  // kernel's prologue and tile loads overlap the schedule kernel (see griddepcontrol.wait above)
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3((unsigned)v.threads);
+  cfg.dynamicSmemBytes = (size_t)smem_bytes;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, f, p, tab);
 }
 
 }  // namespace layup
