@@ -347,3 +347,31 @@ def test_layer_larger_than_2_to_31_elements():
     lu.close()
     del lu, x, g
     torch.cuda.empty_cache()
+
+
+def test_device_schedule_against_curand_directly(curand_pin):
+    """The kernels' own Philox pinned to cuRAND's library routine without going through the oracle:
+    peers and straggler mask drawn ON THE DEVICE (layup_schedule) must equal the values derived from
+    curand_Philox4x32_10 for counter (step, layer | 0xFFFFFFFF, replica, tag) and key = seed."""
+    def words(seed, ctrs):
+        ctr = np.ascontiguousarray(ctrs, dtype=np.uint32)
+        key = np.tile(np.array([seed & 0xFFFFFFFF, seed >> 32], dtype=np.uint32), (ctr.shape[0], 1))
+        out = np.empty_like(ctr)
+        curand_pin.curand_philox_host(ctr.ctypes.data, key.ctypes.data, out.ctypes.data, ctr.shape[0])
+        return out[:, 0].astype(np.uint64)
+
+    for K, L, seed, p, mode in [(8, 5, 0x1234567_89ABCDEF, 0.25, 0), (64, 3, 7, 0.0, 0), (33, 4, 2**63 + 11, 0.5, 1)]:
+        lu = LayUp(K, [64] * L, 0.1, 0.0, seed, mode, p)
+        thr = min(int(float(np.float32(p)) * 4294967296.0), 0xFFFFFFFF)
+        for step in (0, 1, 77, 2**32 - 1):
+            peer, active = lu.layup_schedule(step)
+            skip = words(seed, [(step, 0xFFFFFFFF, i, 1) for i in range(K)])
+            want_active = (skip >= thr) if p > 0 else np.ones(K, dtype=bool)
+            assert np.array_equal(active.astype(bool), want_active)
+            for l in range(L):
+                r = words(seed, [(step, l if mode == 0 else 0xFFFFFFFF, i, 0) for i in range(K)])
+                q = (r * np.uint64(K - 1)) >> np.uint64(32)
+                want = (q + (q >= np.arange(K, dtype=np.uint64))).astype(np.int64)
+                want = np.where(want_active, want, -1)
+                assert np.array_equal(peer[l].astype(np.int64), want), (K, step, l)
+        lu.close()
