@@ -43,6 +43,8 @@ struct layup_ctx {
   SchedTables t{};
   int32_t *d_peer_scratch = nullptr, *d_ticket = nullptr;
   void *d_tmaps = nullptr;                // [n_sections][L] CUtensorMap: 2-D tiled view [K][pad] of every layer section
+  bool ps_ok = false;                     // LAYUP_PERSISTENT=1: persistent two-stage form of the TMA kernel
+  int ps_smem = 0, ps_ctas = 0;
   bool pdl = true;                        // programmatic dependent launch of the update kernel behind the schedule kernel
   bool fused_ok = false;                  // the single-launch path exists for this ctx (K, engine, variant)
   long long fused_max_tiles = 0;          // ... and is taken by launches of at most this many work items
@@ -300,6 +302,16 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
       CU_TRY_INIT(cudaMemcpy(ctx->d_tmaps, maps.data(), sizeof(CUtensorMap) * maps.size(), cudaMemcpyHostToDevice));
     }
   }
+  if (ctx->engine == 1 && ctx->launch_shape == 1 && ctx->mix_mode != kMixSymmetric && ctx->skip_thr == 0u &&
+      ctx->delay_rounds == 0) {
+    ctx->ps_smem = (int)persist_smem_bytes(K, C, ctx->opt);
+    if ((size_t)ctx->ps_smem <= prop.sharedMemPerBlockOptin) {
+      CU_TRY_INIT(persist_kernel_setup(ctx->opt, ctx->ps_smem, &ctx->ps_ctas));
+      const int cap_ps = env_int("LAYUP_CTAS_PER_SM", 0);
+      if (cap_ps > 0 && cap_ps < ctx->ps_ctas) ctx->ps_ctas = cap_ps;
+      ctx->ps_ok = ctx->ps_ctas >= 1;
+    }
+  }
   CU_TRY_INIT(cudaMemcpy(ctx->d_layers, ctx->layers.data(), sizeof(LayerDesc) * L, cudaMemcpyHostToDevice));
   CU_TRY_INIT(cudaMemcpy(ctx->d_tile_prefix, ctx->tile_prefix.data(), sizeof(long long) * (L + 1), cudaMemcpyHostToDevice));
   std::vector<double> w0((size_t)L * K, 1.0 / (double)K);              // PAPER.md:106  w_i = 1/M
@@ -405,7 +417,12 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
       tab.prefix[n] = ctx->tile_prefix[q0 + n] - t0;
       tab.n = n;
       // only the first update launch directly follows the schedule kernel on the stream
-      CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, fused, ctx->pdl && n_launch == 0, (int)tab.prefix[n], ctx->smem, s));
+      if (ctx->ps_ok && !fused) {
+        const int grid = (int)std::min<long long>(tab.prefix[n], (long long)ctx->n_sm * ctx->ps_ctas);
+        CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->pdl && n_launch == 0, s));
+      } else {
+        CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, fused, ctx->pdl && n_launch == 0, (int)tab.prefix[n], ctx->smem, s));
+      }
       q0 += n;
       ++n_launch;
     }

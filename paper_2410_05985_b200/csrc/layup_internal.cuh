@@ -105,4 +105,10 @@ cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_byte
 cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, bool pdl, int grid,
                               int smem_bytes, cudaStream_t s);
 
+// update_persist.cu -- persistent two-stage form (LAYUP_PERSISTENT=1)
+size_t persist_smem_bytes(int K, int C, int opt);
+cudaError_t persist_kernel_setup(int opt, int smem_bytes, int *ctas_per_sm);
+cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, int grid, int smem_bytes, bool pdl,
+                                  cudaStream_t s);
+
 }  // namespace layup

@@ -313,3 +313,24 @@ def test_checkpoint_resume_is_bit_identical(opt):
             assert torch.equal(a.view(what, l), b.view(what, l)), (what, l)
     assert np.array_equal(a.layup_weights(), b.layup_weights())
     a.close(); b.close()
+
+
+@pytest.mark.parametrize("K", [1, 3, 8, 16, 64, 100])
+@pytest.mark.parametrize("opt,mix,mu", [(OPT_SGD, MIX_PUSHSUM, 0.0), (OPT_SGD, MIX_LOSSY, 0.9), (OPT_ADAMW, MIX_PUSHSUM, 0.0)])
+def test_persistent_form_equals_grouped_form(K, opt, mix, mu, monkeypatch):
+    """LAYUP_PERSISTENT=1: resident CTAs drain the work list through a two-stage TMA pipeline.
+    Same bits as the one-CTA-per-work-item launch and as the oracle (LAYUP_FUSED=0 keeps these small
+    launches off the single-launch path so that the persistent kernel is the one that runs; a small
+    CTA cap forces every CTA through many tiles and several layers)."""
+    kw = ADAM if opt == OPT_ADAMW else {}
+    monkeypatch.setenv("LAYUP_FUSED", "0")
+    outs = []
+    for persistent in ("1", "0"):
+        monkeypatch.setenv("LAYUP_PERSISTENT", persistent)
+        monkeypatch.setenv("LAYUP_CTAS_PER_SM", "1")
+        w, lu, ref, _ = _pair(K, NUMEL + [300000], 1e-3, mu, 61 + K, 0.0, opt, mix, **kw)
+        _run(w, lu, ref, None, 3)
+        outs.append([lu.view(WHAT_X, l).cpu().numpy().copy() for l in range(w.L)] + [lu.layup_weights()])
+        lu.close()
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
