@@ -170,16 +170,8 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   while ((long long)cfg->K * C * 2 <= items_target && C < 4096) C *= 2;
   if (items_env <= 0)
     while (C < 64 && (long long)cfg->K * (2 * C) * 16 * ctx->n_sections <= 112 * 1024) C *= 2;
-  if (items_env <= 0) {
-    // a whole round of fewer work items than ~4 per SM is latency bound: smaller tiles, more CTAs
-    // (B200: 148 SMs; chunks stay >= 256 B per replica)
-    auto round_tiles = [&](int c) {
-      long long t = 0;
-      for (int l = 0; l < cfg->L; ++l) t += (pad32(cfg->numel[l]) / 4 + c - 1) / c;
-      return t;
-    };
-    while (C > 16 && round_tiles(C) < 4 * 148) C /= 2;
-  }
+  // (smaller tiles for rounds of only a few work items per SM were tried: more CTAs repeating the
+  //  fused schedule stage made configs[0] slower, 6.2 -> 8.2 us per round.)
   ctx->C = C;
   ctx->log2C = 0;
   while ((1 << ctx->log2C) < C) ++ctx->log2C;
