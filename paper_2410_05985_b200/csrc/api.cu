@@ -35,6 +35,7 @@ struct layup_ctx {
   int engine = 1;                                      // 1: TMA-staged kernel, 0: LDG kernel
   int32_t delay_replica = 0, delay_rounds = 0;
   int diag_C = 0, diag_log2C = 0, diag_smem = 0, diag_ctas = 1;
+  bool diag_two_stage = true;
   double *d_dist = nullptr;
   // device tables
   LayerDesc *d_layers = nullptr;
@@ -574,11 +575,14 @@ extern "C" int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist
   if (ctx->diag_C == 0) {
     // read-only tile: ~2048 float4 items (32 KB) of x per work item
     int C = 8;
-    while ((long long)K * C * 2 <= 2048 && C < 1024) C *= 2;
+    while ((long long)K * C * 2 <= 2048 && C < 256) C *= 2;       // C divides the 256 threads of the kernel
     ctx->diag_C = C;
     while ((1 << ctx->diag_log2C) < C) ++ctx->diag_log2C;
-    ctx->diag_smem = (int)diag_smem_bytes(K, C);
-    CU_TRY(ctx, diag_setup(ctx->diag_smem, &ctx->diag_ctas));
+    cudaDeviceProp prop;
+    CU_TRY(ctx, cudaGetDeviceProperties(&prop, ctx->device));
+    ctx->diag_two_stage = diag_smem_bytes(K, C, true) <= prop.sharedMemPerBlockOptin;   // else one stage (K > ~880)
+    ctx->diag_smem = (int)diag_smem_bytes(K, C, ctx->diag_two_stage);
+    CU_TRY(ctx, diag_setup(K, C, ctx->diag_smem, &ctx->diag_ctas));
     if (ctx->diag_ctas < 1) return fail(ctx, LAYUP_EINVAL, "K=%d does not fit the diagnostic kernel", K);
   }
   cudaStream_t s = ctx->own_stream;
@@ -599,7 +603,7 @@ extern "C" int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist
     const long long tiles = tab.prefix[n];
     const int grid = (int)std::min<long long>(tiles, (long long)ctx->n_sm * ctx->diag_ctas);
     CU_TRY(ctx, launch_disagreement(ctx->arena, weighted ? ctx->d_w : nullptr, ctx->d_dist, K, C, ctx->diag_log2C,
-                                    tab, grid, ctx->diag_smem, s));
+                                    ctx->diag_two_stage, tab, grid, ctx->diag_smem, s));
     ctx->launches += 1;
     q0 += n;
   }

@@ -87,9 +87,9 @@ cudaError_t launch_peers_only(uint64_t seed, uint32_t step, uint32_t skip_thr, i
                               int delay_replica, int delay_rounds, int32_t *peer_dev, unsigned char *active_dev,
                               cudaStream_t s);
 // diagnose.cu
-size_t diag_smem_bytes(int K, int C);
-cudaError_t diag_setup(int smem_bytes, int *ctas_per_sm);
-cudaError_t launch_disagreement(const float *x, const double *w, double *dist, int K, int C, int log2C,
+size_t diag_smem_bytes(int K, int C, bool two_stage);
+cudaError_t diag_setup(int K, int C, int smem_bytes, int *ctas_per_sm);
+cudaError_t launch_disagreement(const float *x, const double *w, double *dist, int K, int C, int log2C, bool two_stage,
                                 const PosTable &tab, int grid, int smem_bytes, cudaStream_t s);
 // update.cu
 int update_num_variants();

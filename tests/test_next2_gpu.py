@@ -41,7 +41,7 @@ def test_delay_mode_parity(K, r, n, p):
     lu.close()
 
 
-@pytest.mark.parametrize("K", [1, 2, 3, 8, 16, 64, 200])
+@pytest.mark.parametrize("K", [1, 2, 3, 8, 16, 64, 200, 1000])
 def test_disagreement_parity(K):
     numel = [1, 33, 1000, 4097, 70001 if K <= 16 else 2049]
     w = synth.Workload("dis", K, tuple(numel), lr=0.05, momentum=0.0, rounds=3, seed=5 + K, grad_std=1e-2)
