@@ -2,7 +2,8 @@
 """bench.py -- param-updates/s and effective HBM GB/s of the LayUp update+gossip round.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME|all] [--impl ours|reference]
-                  [--optimizer sgd|adamw] [--mix pushsum|lossy|symmetric] [--mode round|layers]
+                  [--optimizer sgd|adamw] [--mix pushsum|lossy|symmetric] [--mode round|layers|graph]
+                  [--tuning key=value,...] [--no-per-config]
 
 A "step" is one layup_round(): the whole hot path (straggler mask, peer choice, push-sum
 weights, local step, push, peer mix, reverse-layer work list) over all K replicas of all
@@ -10,7 +11,10 @@ layers of one synthetic batch of gradients.  Default workload = BASELINE.json:co
 (K=16 replicas of the GPT-2-medium parameter set, fp32 + momentum), the largest config
 and the one north_star's bandwidth target is stated on.
 
-Prints ONE JSON line.  N > 1 (torchrun): the path does not shard (north_star: "no
+Prints ONE JSON line; its "per_config" list carries the same measurement (ms per round,
+param-updates/s, effective GB/s, launches) for all five BASELINE configs, the L2-resident ones
+also replayed from a CUDA graph (layup_graph_*), and "cpu_baseline" times the oracle on all
+host cores (the same source built with -fopenmp) beside the single-threaded figure.  N > 1 (torchrun): the path does not shard (north_star: "no
 sharding across GPUs, no collectives"), so each rank runs an independent replica set
 ("replicas only") and value is the sum over ranks / max time.
 --impl reference times the CPU oracle as it stands on a bounded sample of the workload.
@@ -53,9 +57,21 @@ def parse():
                     help="mixer: push-sum fold [default, BASELINE.json], contention-lossy or symmetric (NEXT-4)")
     ap.add_argument("--skip-prob", type=float, default=None,
                     help="override the workload's straggler probability (configs[3] semantics on any shape)")
-    ap.add_argument("--mode", default="round", choices=["round", "layers"],
-                    help="round: one persistent launch per step; layers: L per-layer launches on 4 streams")
+    ap.add_argument("--mode", default="round", choices=["round", "layers", "graph"],
+                    help="round: one layup_round per step (one reverse-layer work list); layers: L per-layer "
+                         "launches on 4 streams; graph: all timed rounds recorded once with layup_graph_* and replayed")
+    ap.add_argument("--tuning", default="", help="layup_tuning fields, e.g. launch_shape=2,stages=4 (include/layup.h)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config list (all five BASELINE configs)")
+    ap.add_argument("--per-config-steps", type=int, default=0, help="timed rounds per config in per_config (0: the config's own round count, at most 20)")
     return ap.parse_args()
+
+
+def tuning_dict(args):
+    out = {}
+    for kv in filter(None, args.tuning.split(",")):
+        k, v = kv.split("=")
+        out[k.strip()] = int(v)
+    return out or None
 
 
 def get_workload(name):
@@ -108,11 +124,13 @@ def committed_traffic(name, optimizer="sgd"):
 
 
 # ---- oracle sample (cpu_baseline and --impl reference) -------------------------------
-def oracle_sample(w, seconds, steps=None, warmup=0, args=None):
-    """Times oracle/ as it stands, single-threaded, on a bounded sample of the workload:
-    the LAST layers of the layer list (output side first, as the path walks them) up to a
-    budget of parameter updates per round."""
+def oracle_sample(w, seconds, steps=None, warmup=0, args=None, all_cores=False):
+    """Times oracle/ as it stands on a bounded sample of the workload: the LAST layers of the
+    layer list (output side first, as the path walks them) up to a budget of parameter updates
+    per round.  all_cores: the same source built with -fopenmp (element loops on every host
+    core, bit-identical results); else the default single-threaded build."""
     import oracle
+    oracle.use_omp(all_cores)
     budget = 200e6                       # param-updates per round in the sample
     layers, tot = [], 0
     for l in reversed(range(w.L)):
@@ -147,22 +165,34 @@ def oracle_sample(w, seconds, steps=None, warmup=0, args=None):
         elif t_used >= seconds or done >= 50:
             break
     ups = sum(per_step_updates) / t_used
-    sample = "layers %d..%d of %d (%.1fM params/replica, K=%d), %d rounds, single thread" % (
-        layers[0], layers[-1], w.L, sum(sub.numel) / 1e6, sub.K, done)
+    oracle.use_omp(False)
+    sample = "layers %d..%d of %d (%.1fM params/replica, K=%d), %d rounds, %s" % (
+        layers[0], layers[-1], w.L, sum(sub.numel) / 1e6, sub.K, done,
+        "OpenMP over elements, %d threads" % (os.cpu_count() or 1) if all_cores else "single thread")
     return ups, t_used / done, sample, sum(per_step_updates) / done
+
+
+def cpu_baseline(w, args):
+    """The oracle on the box's host cores: all cores (reported value) and one thread beside it."""
+    half = args.cpu_seconds / 2
+    a_ups, _, a_sample, _ = oracle_sample(w, half, args=args, all_cores=True)
+    s_ups, _, s_sample, _ = oracle_sample(w, half, args=args, all_cores=False)
+    return {"value": a_ups, "unit": UNIT, "cores": os.cpu_count() or 1, "kind": "oracle", "sample": a_sample,
+            "single_thread": {"value": s_ups, "cores": 1, "sample": s_sample}}
 
 
 def run_reference(args, w, rank, world):
     if rank != 0:
         return
-    ups, s_per_step, sample, _ = oracle_sample(w, args.cpu_seconds, steps=args.steps, warmup=min(args.warmup, 1), args=args)
+    ups, s_per_step, sample, _ = oracle_sample(w, args.cpu_seconds, steps=args.steps, warmup=min(args.warmup, 1), args=args,
+                                               all_cores=True)
     line = {
         "metric": METRIC, "value": ups, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": s_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic", "impl": "reference",
         "config": {"workload": "%s (%s)" % (w.name, w.note), "K": w.K, "L": w.L,
                    "params_per_replica": w.params_per_replica, "momentum": w.momentum},
-        "cpu_baseline": {"value": ups, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": ups, "unit": UNIT, "cores": os.cpu_count() or 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": ups, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -242,8 +272,121 @@ def reduce_over_ranks(dist, ms, updates, nbytes, device):
     return float(t.item()), float(tot[0].item()), float(tot[1].item())
 
 
+class Timed:
+    """One timed run of `steps` rounds on a fresh ctx: CUDA events on the launching stream around the
+    whole sequence (ms), the library's own event pairs around every launching call (kernel_ms)."""
+
+    def __init__(self, args, w, rank, local_rank, mode, barrier):
+        from paper_2410_05985_b200 import WHAT_G, WHAT_X, LayUp
+        self.w, self.mode, self.args = w, mode, args
+        mom = 0.0 if args.optimizer == "adamw" else w.momentum
+        self.lu = lu = LayUp(w.K, w.numel, w.lr, mom, w.seed + 1000 * rank, w.peer_mode, w.skip_prob, device=local_rank,
+                             tuning=tuning_dict(args), **rule_kwargs(args))
+        for l in range(w.L):
+            synth.fill_init_(w, l, lu.view(WHAT_X, l))
+            synth.fill_grad_(w, 0, l, lu.view(WHAT_G, l), data_seed=w.seed + 1000 * rank)
+        torch.cuda.synchronize()
+        self.streams = [torch.cuda.Stream() for _ in range(4)] if mode == "layers" else None
+        self.step = 0
+        self.barrier = barrier
+
+    def one_step(self):
+        lu, w, s = self.lu, self.w, self.step
+        if self.mode == "layers":
+            for k, l in enumerate(reversed(range(w.L))):
+                lu.layup_layer_update(s, l, self.streams[k % 4])
+        else:
+            lu.layup_round(s)
+        self.step += 1
+
+    def run(self, steps, warmup):
+        lu, w = self.lu, self.w
+        for _ in range(warmup):
+            self.one_step()
+        lu.layup_sync()
+        graph = gstream = None
+        if self.mode == "graph":
+            # all timed rounds recorded once (the round counter is device state), then one replay to warm up
+            gstream = torch.cuda.Stream()
+            lu.layup_graph_begin(gstream)
+            for r in range(steps):
+                lu.layup_round(self.step + r, gstream)
+            graph = lu.layup_graph_end()
+            lu.layup_graph_launch(graph, gstream)
+            self.step += steps
+            lu.layup_sync()
+        launches0 = lu.layup_launch_count()
+        lu.layup_profile(self.mode != "graph")
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        self.barrier()
+        self.t0 = time.perf_counter()
+        self.first = self.step
+        cur = torch.cuda.current_stream()
+        for st in (self.streams or []) + ([gstream] if gstream else []):
+            st.wait_stream(cur)
+        tstream = gstream or cur
+        ev0.record(tstream)
+        if graph is not None:
+            lu.layup_graph_launch(graph, gstream)
+            self.step += steps
+        else:
+            for _ in range(steps):
+                self.one_step()
+        for st in (self.streams or []):
+            cur.wait_stream(st)
+        ev1.record(tstream)
+        self.barrier()
+        self.t1 = time.perf_counter()
+        ms = ev0.elapsed_time(ev1)
+        n_k, k_ms = lu.layup_profile_read()
+        lu.layup_profile(False)
+        launches = lu.layup_launch_count() - launches0
+        if graph is not None:
+            lu.layup_graph_destroy(graph)
+        bts, ups = algorithmic_bytes(w, lu, range(self.first, self.first + steps), self.args)
+        return dict(ms=ms, steps=steps, launches=launches, n_k=n_k, k_ms=k_ms, bytes=sum(bts), updates=sum(ups))
+
+    def close(self):
+        self.lu.close()
+        del self.lu
+        torch.cuda.empty_cache()
+
+
+def per_config_report(args, rank, local_rank, barrier, main_name, main_entry):
+    """north_star "Report per config": every BASELINE config under the same clock.  The L2-resident
+    configs are also replayed from a CUDA graph (launch-latency path)."""
+    out = []
+    for w in synth.workloads():
+        if w.name == main_name:
+            out.append(main_entry)
+            continue
+        steps = args.per_config_steps or min(w.rounds, 20)
+        small = w.K * w.params_per_replica * 12 < 126e6
+        for mode in (["round", "graph"] if small else ["round"]):
+            try:
+                t = Timed(args, w, rank, local_rank, mode, barrier)
+                r = t.run(steps, max(args.warmup, 3))
+                t.close()
+                out.append(config_entry(w, mode, r))
+            except Exception as ex:                      # e.g. not enough HBM next to the main arena
+                out.append({"workload": w.name, "mode": mode, "error": str(ex)[:200]})
+    return out
+
+
+def config_entry(w, mode, r):
+    ms = r["ms"] / r["steps"]
+    gbs = r["bytes"] / r["steps"] / (ms * 1e-3) / 1e9
+    e = {"workload": "%s (%s)" % (w.name, w.note), "K": w.K, "L": w.L, "mode": mode, "rounds_timed": r["steps"],
+         "ms_per_round": ms, "param_updates_per_s": r["updates"] / (r["ms"] * 1e-3), "effective_hbm_gbs": gbs,
+         "frac_of_8TBs_nominal": gbs / 8000.0, "launches_per_round": r["launches"] / r["steps"],
+         "l2": "inputs larger than L2" if r["bytes"] / r["steps"] > 4 * 126e6 else "L2-resident (launch-latency bound)"}
+    if r["n_k"]:
+        e["kernel_ms_per_round"] = r["k_ms"] / r["steps"]
+    return e
+
+
 def run_ours(args, w, rank, world, local_rank):
-    from paper_2410_05985_b200 import WHAT_G, WHAT_X, LayUp
+    from paper_2410_05985_b200 import WHAT_G
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local_rank)
     dist = None
@@ -257,66 +400,47 @@ def run_ours(args, w, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
-    mom = 0.0 if args.optimizer == "adamw" else w.momentum
-    lu = LayUp(w.K, w.numel, w.lr, mom, w.seed + 1000 * rank, w.peer_mode, w.skip_prob, device=local_rank,
-               **rule_kwargs(args))
-    for l in range(w.L):
-        synth.fill_init_(w, l, lu.view(WHAT_X, l))
-        synth.fill_grad_(w, 0, l, lu.view(WHAT_G, l), data_seed=w.seed + 1000 * rank)
-    torch.cuda.synchronize()
-    streams = [torch.cuda.Stream() for _ in range(4)] if args.mode == "layers" else None
-
-    def one_step(s):
-        if args.mode == "round":
-            lu.layup_round(s)
-        else:
-            for k, l in enumerate(reversed(range(w.L))):
-                lu.layup_layer_update(s, l, streams[k % 4])
-
-    step = 0
-    for _ in range(args.warmup):
-        one_step(step); step += 1
-    lu.layup_sync()
-    launches0 = lu.layup_launch_count()
-    lu.layup_profile(True)
+    timed = Timed(args, w, rank, local_rank, args.mode, barrier)
+    lu = timed.lu
     sampler = ClockSampler(local_rank) if rank == 0 else None
     time.sleep(0.3)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    t0 = time.perf_counter()
-    first = step
-    if streams:
-        for st in streams:
-            st.wait_stream(torch.cuda.current_stream())
-    ev0.record()
-    for _ in range(args.steps):
-        one_step(step); step += 1
-    if streams:
-        for st in streams:
-            torch.cuda.current_stream().wait_stream(st)
-    ev1.record()
-    barrier()
-    t1 = time.perf_counter()
-    ms = ev0.elapsed_time(ev1)
-    n_k, k_ms = lu.layup_profile_read()
-    lu.layup_profile(False)
-    launches = lu.layup_launch_count() - launches0
-    clocks = sampler.summary(t0, t1) if sampler else None
-    bts, ups = algorithmic_bytes(w, lu, range(first, first + args.steps), args)
+    r = timed.run(args.steps, args.warmup)
+    clocks = sampler.summary(timed.t0, timed.t1) if sampler else None
+    step = timed.step
+    n_k, k_ms, launches = r["n_k"], r["k_ms"], r["launches"]
 
-    ms, job_updates, job_bytes = reduce_over_ranks(dist, ms, sum(ups), sum(bts), torch.device("cuda", local_rank))
+    ms, job_updates, job_bytes = reduce_over_ranks(dist, r["ms"], r["updates"], r["bytes"], torch.device("cuda", local_rank))
     value = job_updates / (ms * 1e-3)
     eff_gbs = job_bytes / (ms * 1e-3) / 1e9
 
     # ---- roofline of the dominant kernel (the fused update kernel), this rank
     peak, peak_src = measured_peak()
-    k_avg_ms = k_ms / max(n_k, 1)
-    bytes_per_launch = sum(bts) / max(n_k, 1)
+    if n_k:
+        k_avg_ms = k_ms / n_k
+        bytes_per_launch = r["bytes"] / n_k
+    else:                                                # graph replay: the whole sequence is one timed launch
+        k_avg_ms, bytes_per_launch = r["ms"] / args.steps, r["bytes"] / args.steps
     achieved = bytes_per_launch / (k_avg_ms * 1e-3) / 1e9 if k_avg_ms > 0 else 0.0
+    kernel = "layup_update_persist" if (tuning_dict(args) or {}).get("launch_shape") == 2 else "layup_update_tma"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": committed_traffic(w.name, args.optimizer) if args.mix == "pushsum" else None, "kernel": "layup_update_tma",
+                "traffic": committed_traffic(w.name, args.optimizer) if args.mix == "pushsum" and kernel == "layup_update_tma" else None,
+                "kernel": kernel,
                 "kernel_ms_avg": k_avg_ms, "kernel_launches": n_k, "algorithmic_bytes_per_launch": bytes_per_launch,
                 "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0}
+
+    # ---- the read-only diagnostic kernel of the path (layup_disagreement), device time
+    diag = None
+    try:
+        lu.layup_disagreement(False)
+        d_ms = []
+        for _ in range(3):
+            lu.layup_disagreement(False)
+            d_ms.append(lu.layup_disagreement_ms())
+        d = float(np.median(d_ms))
+        diag = {"kernel": "layup_disagreement_kernel", "ms": d, "read_gbs": 4.0 * w.K * w.params_per_replica / (d * 1e-3) / 1e9,
+                "frac_of_measured_peak": 4.0 * w.K * w.params_per_replica / (d * 1e-3) / 1e9 / peak}
+    except Exception as ex:
+        diag = {"error": str(ex)[:200]}
 
     # ---- e2e: same metric through the C-ABI with HOST buffers (h2d grads + d2h params in the timed region)
     e2e = None
@@ -350,25 +474,31 @@ def run_ours(args, w, rank, world, local_rank):
         except Exception as ex:                  # e.g. the box cannot pin 2 x K x N x 4 bytes
             e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
     lu.layup_sync()
+    main_entry = config_entry(w, args.mode, r)
+    timed.close()
+
+    per_config = None
+    if not args.no_per_config and world == 1 and args.config == "gpt2m_k16":
+        per_config = per_config_report(args, rank, local_rank, barrier, w.name, main_entry)
 
     if rank != 0:
         return
     cpu = None
     if not args.no_cpu_baseline and world == 1:
-        c_ups, _, sample, _ = oracle_sample(w, args.cpu_seconds, args=args)
-        cpu = {"value": c_ups, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
-               "host_cores": os.cpu_count()}
+        cpu = cpu_baseline(w, args)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "%s (%s)" % (w.name, w.note), "K": w.K, "L": w.L,
                    "params_per_replica": w.params_per_replica, "momentum": w.momentum, "lr": w.lr,
-                   "skip_prob": w.skip_prob, "mode": args.mode, "optimizer": args.optimizer, "mix": args.mix, "parallelism": "replicas only x%d" % world,
+                   "skip_prob": w.skip_prob, "mode": args.mode, "optimizer": args.optimizer, "mix": args.mix,
+                   "tuning": tuning_dict(args), "parallelism": "replicas only x%d" % world,
                    "l2": "inputs larger than L2" if job_bytes / args.steps / world > 4 * 126e6 else
                          "L2-resident working set (launch-latency bound, see DESIGN.md)"},
         "effective_hbm_gbs": eff_gbs, "frac_of_8TBs_nominal": eff_gbs / world / 8000.0,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "diagnostic": diag, "per_config": per_config,
     }
     print(json.dumps(line), flush=True)
 
@@ -389,7 +519,6 @@ def main():
             run_reference(args, w, rank, world)
         else:
             run_ours(args, w, rank, world, local_rank)
-            torch.cuda.empty_cache()
     if world > 1 and args.impl != "reference":
         import torch.distributed as dist
         if dist.is_initialized():

@@ -20,7 +20,8 @@
  *    them alive until layup_destroy(); the library borrows them.  It owns only its small
  *    tables (layer table, schedule tables, weights w[L][K]); it never allocates
  *    parameter-sized memory ("without buffering").
- *  - A ctx is used from one host thread at a time.
+ *  - A ctx is used from one host thread at a time.  Every call leaves the calling thread's
+ *    current CUDA device as it found it.
  *  - There is no CPU fallback: without a CUDA device every launching call fails with
  *    LAYUP_ECUDA.
  *
@@ -63,7 +64,31 @@ extern "C" {
 
 #define LAYUP_MAX_K 1024  /* replicas (workers) per ctx                               */
 
-typedef struct layup_ctx layup_ctx;   /* opaque */
+typedef struct layup_ctx layup_ctx;       /* opaque */
+typedef struct layup_graph layup_graph;   /* opaque: a captured sequence of launching calls */
+
+/* Launch tuning, all optional: 0 in a field = the library's default, and a NULL pointer in
+ * layup_config.tuning = all defaults.  None of them changes a single result bit (every launch
+ * shape is parity-tested against the oracle); they select WHICH of the library's kernels runs.
+ * This block is the only switch: the library reads no environment variable. */
+typedef struct {
+  int32_t engine;       /* 0 auto: TMA-staged kernel while the tile of all K replicas fits in shared
+                           memory, else the LDG kernel; 1 TMA-staged; 2 LDG                         */
+  int32_t launch_shape; /* 0 auto = 1; 1 grouped: one CTA per (layer, tile) work item, the list in
+                           reverse layer order; 2 persistent: resident CTAs drain the same list
+                           through a multi-stage TMA ring                             */
+  int32_t fused;        /* 0 auto = 1; 1: launches of at most fused_waves waves of work items run the
+                           schedule stage inside the update kernel (ONE launch); 2: never            */
+  int32_t fused_waves;  /* default 4                                                                */
+  int32_t tile_items;   /* float4 items (replicas x columns) per work item; default 1024            */
+  int32_t variant;      /* thread shape of the update kernel: 0 default, 1.. alternatives + 1       */
+  int32_t ctas_per_sm;  /* cap on resident CTAs per SM of persistent grids; default: all that fit   */
+  int32_t pdl;          /* 0 auto = 1; 1: the update kernel is a programmatic dependent launch behind
+                           the schedule kernel; 2: plain stream order                               */
+  int32_t tma2d;        /* 0 auto (by K and optimiser); 1: one 2-D tiled TMA load per
+                           array and tile; 2: K 1-D bulk copies per array and tile                  */
+  int32_t stages;       /* persistent shape: depth of the TMA ring; default: as deep as fits        */
+} layup_tuning;
 
 typedef struct {
   int32_t  K;          /* workers M of the paper, 1 <= K <= LAYUP_MAX_K    */
@@ -87,6 +112,7 @@ typedef struct {
   float    beta1;      /* AdamW only: 0 <= beta1 < 1                                       */
   float    beta2;      /* AdamW only: 0 <= beta2 < 1                                       */
   float    eps;        /* AdamW only: >= 0                                                 */
+  const layup_tuning *tuning; /* HOST, may be NULL (defaults); read during layup_init only         */
 } layup_config;
 
 /* Bytes of device memory the arena needs for this config (X + G (+ M (+ V)), padded). Pure. */
@@ -117,8 +143,12 @@ int layup_set_lr(layup_ctx *ctx, float lr);
  * (PAPER.md:23,25).  cuda_stream: a cudaStream_t (NULL = legacy default stream). */
 int layup_layer_update(layup_ctx *ctx, int64_t step, int32_t layer, void *cuda_stream);
 
-/* All layers L-1 .. 0 of round `step` in one persistent grouped launch that drains a
- * reverse-layer-ordered work list.  Bit-identical to L calls of layup_layer_update. */
+/* All layers L-1 .. 0 of round `step` as ONE work list in reverse layer order:
+ * by default a grouped launch, one CTA per (layer, tile) work item, which the hardware CTA
+ * scheduler drains in list order (two kernels: schedule stage + update; one kernel when the
+ * launch is small, see layup_tuning.fused; lists of more than 160 layers are split into
+ * consecutive launches); with layup_tuning.launch_shape = 2 a persistent kernel whose resident
+ * CTAs walk the same list.  Bit-identical to L calls of layup_layer_update. */
 int layup_round(layup_ctx *ctx, int64_t step, void *cuda_stream);
 
 /* layup_round with HOST buffers, layer-pipelined: for l = L-1..0 copy layer l's
@@ -126,7 +156,10 @@ int layup_round(layup_ctx *ctx, int64_t step, void *cuda_stream);
  * stages of consecutive layers overlapping on the library's own streams.
  * g_host, x_host: [sum_l K*numel[l]] fp32, layer-major then replica (no padding), should
  * be pinned for the copies to be asynchronous; x_host may be NULL (no read-back).
- * Returns after the last copy has completed (synchronous). */
+ * Returns after the last copy has completed (synchronous).  The step bookkeeping is committed
+ * only when the whole round succeeded; on a mid-round CUDA failure the library first waits for
+ * its copy streams (the host buffers are no longer in use when the call returns), and the ctx
+ * is POISONED: every later launching call returns LAYUP_ECUDA (the arena holds a partial round). */
 int layup_round_host(layup_ctx *ctx, int64_t step, const float *g_host, float *x_host);
 
 /* Wait for every stream the ctx has launched on; report the first sticky CUDA error. */
@@ -140,9 +173,39 @@ int layup_sync(layup_ctx *ctx);
 int layup_peer(uint64_t seed, int64_t step, int32_t layer, int32_t replica, int32_t K,
                int32_t *peer);
 
-/* Runs the DEVICE schedule stage for round `step` without touching any state and copies
- * it out: peer[l*K+i] (-1 if replica i is inactive) and active[i].  Synchronous. */
+/* The peer choice and straggler mask of an ARBITRARY round `step`, drawn on the device by a
+ * read-only kernel (the same draw_peer / draw_active device functions the schedule stage calls;
+ * no state touched): peer[l*K+i] (-1 if replica i is inactive) and active[i].  What the update
+ * kernel actually consumed in the last issued round is layup_schedule_tables().  Synchronous. */
 int layup_schedule(layup_ctx *ctx, int64_t step, int32_t *peer /*[L*K]*/, uint8_t *active /*[K]*/);
+
+/* The schedule tables the update kernel CONSUMED for the most recent (step, layer) event of
+ * `layer`, as the schedule stage left them on the device (two-launch path: written by the
+ * schedule kernel and read by the update kernel; single-launch path: the copy the update kernel
+ * computed in shared memory, written out by the CTA that retires the layer):
+ *   peer[i]      chosen peer of replica i, -1 if inactive
+ *   flags[i]     bit 0: active (local step + push), bit 1: receives >= 1 push
+ *   recv_off[j]  CSR by receiver: entries [recv_off[j], recv_off[j+1]) of senders/alpha
+ *   senders[k]   sender of entry k, ascending within a receiver (R3)
+ *   alpha[k]     w_i/(w_i+w_j) of that push, fp64 divide rounded once to fp32
+ * With the symmetric mixer only peer and flags are meaningful (no sender list).  Any pointer may
+ * be NULL.  step_done receives the step that event applied.  Waits for the ctx's work.  HOST. */
+int layup_schedule_tables(layup_ctx *ctx, int32_t layer, int64_t *step_done, int32_t *peer /*[K]*/,
+                          uint8_t *flags /*[K]*/, int32_t *recv_off /*[K+1]*/, int32_t *senders /*[K]*/,
+                          float *alpha /*[K]*/);
+
+/* Issue order ("output layer first"): the layers of the most recent launching
+ * call in the order the library put them on the device -- the work-list positions of layup_round
+ * / a graph, the per-layer launches of layup_round_host, the single layer of layup_layer_update.
+ * layers: HOST [L]; *n = entries written. */
+int layup_last_order(layup_ctx *ctx, int32_t *layers /*[L]*/, int32_t *n);
+
+/* Device-side evidence of the same order: while enabled, the first CTA of every (step, layer)
+ * event to start records the GPU's nanosecond timer (%globaltimer, atomicMin per layer).
+ * layup_trace(ctx, 1) arms and clears; layup_trace_read copies out first_ns[l] (UINT64_MAX = layer
+ * not started since arming) after waiting for the ctx's work.  HOST array. */
+int layup_trace(layup_ctx *ctx, int32_t enable);
+int layup_trace_read(layup_ctx *ctx, uint64_t *first_ns /*[L]*/);
 
 /* Current push-sum weights w[l*K+i], after all work issued so far. */
 int layup_weights(layup_ctx *ctx, double *w /*[L*K]*/);
@@ -159,8 +222,30 @@ int layup_state_import(layup_ctx *ctx, const double *w, const double *bpow, cons
  * replica i, dist[l*K+i] = sum_e (x_i[e] - xbar[e])^2, where xbar = (1/K) sum_i x_i (weighted == 0,
  * the paper's plain average) or xbar = sum_i w_i x_i with the current push-sum weights
  * (weighted != 0).  Runs a read-only reduction kernel (fp64 accumulation, 4 B of HBM traffic per
- * parameter) after all work issued so far; dist is a HOST array.  Synchronous. */
-int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist /*[L*K]*/);
+ * parameter) on `cuda_stream` -- after everything the ctx has issued so far (the library waits
+ * for its own streams) and in stream order after the caller's own writes to x on that stream --
+ * then copies dist to the HOST array and returns.  Synchronous. */
+int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist /*[L*K]*/, void *cuda_stream);
+/* Device time of the reduction kernel(s) of the last layup_disagreement call (CUDA events). */
+int layup_disagreement_ms(layup_ctx *ctx, double *ms);
+
+/* ---- CUDA-graph capture of launching calls ------------------------------------------ */
+/* The round number is DEVICE state (one counter per layer, read and advanced by the schedule
+ * stage), not a kernel argument, so a recorded sequence of launches can be replayed for later
+ * rounds.  layup_graph_begin puts `cuda_stream` (not the legacy default stream) into capture;
+ * the layup_layer_update / layup_round calls that follow ON THAT STREAM are recorded, not run
+ * (their `step` arguments are checked as usual and count on from the ctx's state);
+ * layup_graph_end closes the capture and instantiates it; layup_graph_launch replays the
+ * recorded (layer) events for whatever rounds come next, advancing the ctx's step bookkeeping
+ * by what was recorded.  The learning rate in force at capture time is baked into the graph
+ * (layup_set_lr needs a new capture).  Typical use: one graph = one backward's worth of
+ * per-layer events, or one or several whole rounds of an L2-resident model, where the launch
+ * overhead, not HBM, is the cost.  layup_sync checks the device counters against
+ * the host's bookkeeping (LAYUP_ESTATE on disagreement). */
+int layup_graph_begin(layup_ctx *ctx, void *cuda_stream);
+int layup_graph_end(layup_ctx *ctx, layup_graph **out);
+int layup_graph_launch(layup_ctx *ctx, layup_graph *g, void *cuda_stream);
+int layup_graph_destroy(layup_ctx *ctx, layup_graph *g);
 
 /* Device time of the path's kernels, measured with CUDA events on the launch stream around
  * every launching call's kernels (the schedule kernel, a few microseconds, and the fused update

@@ -18,47 +18,84 @@ _SO = os.path.join(_HERE, "liblayup_oracle.so")
 _lib = None
 
 
+_CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
+
+
+def _compile(so, extra):
+    if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+        tmp = so + ".tmp.%d" % os.getpid()
+        subprocess.check_call(["gcc"] + _CFLAGS + extra + ["-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, so)
+    return so
+
+
 def build(force=False):
     """gcc -O2 -ffp-contract=off: no contraction the source does not spell as fmaf()."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        tmp = _SO + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
-                               "-o", tmp, _SRC, "-lm"])
-        os.replace(tmp, _SO)
-    return _SO
+    if force and os.path.exists(_SO):
+        os.remove(_SO)
+    return _compile(_SO, [])
+
+
+def build_omp():
+    """The same source and flags plus -fopenmp: the element loops marked ORACLE_PAR run on all host
+    cores (bench.py's all-cores baseline).  Bit-identical to the serial build (tests/test_oracle_omp.py)."""
+    return _compile(os.path.join(_HERE, "liblayup_oracle_omp.so"), ["-fopenmp"])
+
+
+def _declare(L):
+    c = ctypes
+    _lib = L
+    _lib.oracle_philox4x32_10.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p]
+    _lib.oracle_philox4x32_10.restype = None
+    _lib.oracle_active.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_float]
+    _lib.oracle_active.restype = c.c_int32
+    _lib.oracle_peer.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_int32, c.c_int32]
+    _lib.oracle_peer.restype = c.c_int32
+    _lib.oracle_active_ex.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_float, c.c_int32, c.c_int32]
+    _lib.oracle_active_ex.restype = c.c_int32
+    _lib.oracle_schedule.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_int32, c.c_float,
+                                     c.c_int32, c.c_int32, c.c_void_p, c.c_void_p]
+    _lib.oracle_disagreement.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p]
+    _lib.oracle_disagreement.restype = None
+    _lib.oracle_schedule.restype = None
+    for name, ft in (("oracle_layer_update", c.c_float), ("oracle_layer_update_f64", c.c_double)):
+        f = getattr(_lib, name)
+        f.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
+                      ft, ft, c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_int32,
+                      c.c_void_p, c.c_void_p]
+        f.restype = c.c_int
+    for name in ("oracle_layer_update_ex", "oracle_layer_update_ex_f64"):
+        f = getattr(_lib, name)
+        f.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
+                      c.c_void_p, c.c_void_p, c.POINTER(_Opts), c.c_uint64, c.c_int64, c.c_int32, c.c_int32,
+                      c.c_float, c.c_int32, c.c_int32, c.c_void_p, c.c_void_p]
+        f.restype = c.c_int
+    _lib.oracle_mix_tables.argtypes = [c.c_int32, c.c_void_p, c.c_void_p, c.c_void_p, c.c_int32,
+                                       c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+    _lib.oracle_mix_tables.restype = None
+    return L
 
 
 def lib():
     global _lib
     if _lib is None:
-        _lib = ctypes.CDLL(build())
-        c = ctypes
-        _lib.oracle_philox4x32_10.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p]
-        _lib.oracle_philox4x32_10.restype = None
-        _lib.oracle_active.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_float]
-        _lib.oracle_active.restype = c.c_int32
-        _lib.oracle_peer.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_int32, c.c_int32]
-        _lib.oracle_peer.restype = c.c_int32
-        _lib.oracle_active_ex.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_float, c.c_int32, c.c_int32]
-        _lib.oracle_active_ex.restype = c.c_int32
-        _lib.oracle_schedule.argtypes = [c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_int32, c.c_float,
-                                         c.c_int32, c.c_int32, c.c_void_p, c.c_void_p]
-        _lib.oracle_disagreement.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p]
-        _lib.oracle_disagreement.restype = None
-        _lib.oracle_schedule.restype = None
-        for name, ft in (("oracle_layer_update", c.c_float), ("oracle_layer_update_f64", c.c_double)):
-            f = getattr(_lib, name)
-            f.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
-                          ft, ft, c.c_uint64, c.c_int64, c.c_int32, c.c_int32, c.c_float, c.c_int32, c.c_int32,
-                          c.c_void_p, c.c_void_p]
-            f.restype = c.c_int
-        for name in ("oracle_layer_update_ex", "oracle_layer_update_ex_f64"):
-            f = getattr(_lib, name)
-            f.argtypes = [c.c_int32, c.c_int64, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p,
-                          c.c_void_p, c.c_void_p, c.POINTER(_Opts), c.c_uint64, c.c_int64, c.c_int32, c.c_int32,
-                          c.c_float, c.c_int32, c.c_int32, c.c_void_p, c.c_void_p]
-            f.restype = c.c_int
+        _lib = _declare(ctypes.CDLL(build()))
     return _lib
+
+
+_lib_omp = None
+
+
+def use_omp(enable=True):
+    """Route this module's calls through the -fopenmp build of the same source (or back)."""
+    global _lib, _lib_omp
+    if enable:
+        if _lib_omp is None:
+            _lib_omp = _declare(ctypes.CDLL(build_omp()))
+        _lib = _lib_omp
+    else:
+        _lib = None
+        lib()
 
 
 class _Opts(ctypes.Structure):
@@ -102,6 +139,23 @@ def schedule(seed, step, L, K, peer_mode=0, skip_prob=0.0, delay_replica=0, dela
     a = np.empty(K, dtype=np.uint8)
     lib().oracle_schedule(seed, step, L, K, peer_mode, skip_prob, delay_replica, delay_rounds, _ptr(p), _ptr(a))
     return p, a
+
+
+def mix_tables(w, peer, active, mix_mode=0):
+    """-> (recv_off[K+1], senders[n], alpha[n], w_new[K]) for one (step, layer): the sender list of
+    every receiver in ascending order with the coefficient of each push (oracle_mix_tables)."""
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    K = w.shape[0]
+    peer = np.ascontiguousarray(peer, dtype=np.int32)
+    active = np.ascontiguousarray(active, dtype=np.uint8)
+    recv_off = np.zeros(K + 1, dtype=np.int32)
+    senders = np.zeros(K, dtype=np.int32)
+    alpha = np.zeros(K, dtype=np.float32)
+    w_new = np.empty(K, dtype=np.float64)
+    lib().oracle_mix_tables(K, _ptr(w), _ptr(peer), _ptr(active), mix_mode, _ptr(recv_off), _ptr(senders), _ptr(alpha),
+                            _ptr(w_new))
+    n = int(recv_off[K])
+    return recv_off, senders[:n].copy(), alpha[:n].copy(), w_new
 
 
 def disagreement(x, w=None):

@@ -33,11 +33,22 @@
  *
  * Build: gcc -O2 -ffp-contract=off -shared -fPIC (oracle/__init__.py).  All fp32
  * multiply-adds that the rule fuses are written as explicit fmaf().
+ * The default build is single-threaded.  The SAME source built with -fopenmp
+ * (oracle.build_omp(), bench.py's all-cores baseline) runs the element loops marked
+ * ORACLE_PAR on all host cores: elements are independent, the statements and their
+ * order per element are unchanged, so the results are bit-identical (asserted by
+ * tests/test_oracle_omp.py).
  */
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+
+#ifdef _OPENMP
+#define ORACLE_PAR _Pragma("omp parallel for schedule(static) if (n >= 32768)")
+#else
+#define ORACLE_PAR
+#endif
 
 #define TAG_PEER 0u
 #define TAG_SKIP 1u
@@ -205,6 +216,7 @@ int oracle_layer_update_ex(int32_t K, int64_t n, float *x, const float *g, float
     const float *gi = g + (size_t)i * n;
     float *yi = y + (size_t)i * n;
     if (!active[i]) {
+      ORACLE_PAR
       for (int64_t e = 0; e < n; ++e) yi[e] = xi[e];
     } else if (o->optimizer == OPT_ADAMW) {
       /* AdamW (Loshchilov & Hutter), PyTorch's order of operations:
@@ -220,6 +232,7 @@ int oracle_layer_update_ex(int32_t K, int64_t n, float *x, const float *g, float
       tcount[i] += 1;
       const float c1 = (float)((double)lr / (1.0 - bpow[2 * i + 0]));
       const float c2 = (float)(1.0 / sqrt(1.0 - bpow[2 * i + 1]));
+      ORACLE_PAR
       for (int64_t e = 0; e < n; ++e) {
         const float xd = xi[e] * decay;
         const float mm = fmaf(b1, mi[e], omb1 * gi[e]);
@@ -232,6 +245,7 @@ int oracle_layer_update_ex(int32_t K, int64_t n, float *x, const float *g, float
       }
     } else {
       float *mi = mu != 0.0f ? m + (size_t)i * n : NULL;
+      ORACLE_PAR
       for (int64_t e = 0; e < n; ++e) {
         float d = gi[e];
         if (wd != 0.0f) d = fmaf(wd, xi[e], d);      /* coupled decay: d = g + wd*x     */
@@ -251,6 +265,7 @@ int oracle_layer_update_ex(int32_t K, int64_t n, float *x, const float *g, float
     for (int32_t i = 0; i < K; ++i) {
       if (!(active[i] && peer[i] >= 0)) continue;
       float *yi = y + (size_t)i * n, *yj = y + (size_t)peer[i] * n;
+      ORACLE_PAR
       for (int64_t e = 0; e < n; ++e) {
         const float avg = 0.5f * (yi[e] + yj[e]);
         yi[e] = avg;
@@ -267,12 +282,14 @@ int oracle_layer_update_ex(int32_t K, int64_t n, float *x, const float *g, float
       int32_t last = -1;
       for (int32_t i = 0; i < K; ++i)
         if (active[i] && peer[i] == j) last = i;
+      ORACLE_PAR
       for (int64_t e = 0; e < n; ++e) acc[e] = yj[e];
       for (int32_t i = 0; i < K; ++i) {
         if (!(active[i] && peer[i] == j)) continue;
         if (o->mix_mode == MIX_LOSSY && i != last) continue;  /* overwritten: skipped       */
         const float alpha = (float)(wh[i] / (W + wh[i]));   /* w_i/(w_i+w_j), one rounding */
         const float *yi = y + (size_t)i * n;
+        ORACLE_PAR
         for (int64_t e = 0; e < n; ++e) {
           const float d = yi[e] - acc[e];
           acc[e] = fmaf(alpha, d, acc[e]);                  /* = (1-a)*x_j + a*x_i */
@@ -280,6 +297,7 @@ int oracle_layer_update_ex(int32_t K, int64_t n, float *x, const float *g, float
         W = W + wh[i];                                      /* w_j <- w_j + w_i    */
       }
       float *xj = x + (size_t)j * n;
+      ORACLE_PAR
       for (int64_t e = 0; e < n; ++e) xj[e] = acc[e];
       w[j] = W;
     }
@@ -287,6 +305,38 @@ int oracle_layer_update_ex(int32_t K, int64_t n, float *x, const float *g, float
 
   free(peer); free(active); free(wh); free(y); free(acc);
   return 0;
+}
+
+/* ---- the scalar half of steps 2 and 4 on its own: for a given schedule (peer, active) and
+ * weights w, the halved weights, then per receiver j in ascending sender index the coefficient
+ * alpha = w_i/(w_i+w_j) of every push that lands ("Peer Update") and the weight
+ * after it (w_j <- w_j + w_i).  Output as a CSR by receiver: entries [recv_off[j], recv_off[j+1])
+ * of senders[] / alpha[] belong to receiver j.  The statements are those of step 4 of
+ * oracle_layer_update_ex; tests compare this list with the tables the CUDA path consumed
+ * (layup_schedule_tables) and pin it against oracle_layer_update_ex itself.  MIX_SYMMETRIC has no
+ * sender list (recv_off all zero, weights unchanged).                                     */
+void oracle_mix_tables(int32_t K, const double *w, const int32_t *peer, const uint8_t *active, int32_t mix_mode,
+                       int32_t *recv_off, int32_t *senders, float *alpha, double *w_out) {
+  int32_t k = 0;
+  for (int32_t j = 0; j < K; ++j) {
+    const double whj = (active[j] && K >= 2 && mix_mode != MIX_SYMMETRIC) ? w[j] * 0.5 : w[j];
+    double W = whj;
+    recv_off[j] = k;
+    int32_t last = -1;
+    for (int32_t i = 0; i < K; ++i)
+      if (active[i] && peer[i] == j) last = i;
+    for (int32_t i = 0; i < K && mix_mode != MIX_SYMMETRIC; ++i) {
+      if (!(active[i] && peer[i] == j)) continue;
+      if (mix_mode == MIX_LOSSY && i != last) continue;
+      const double whi = w[i] * 0.5;                        /* a sender has halved its weight */
+      senders[k] = i;
+      alpha[k] = (float)(whi / (W + whi));
+      W = W + whi;
+      ++k;
+    }
+    w_out[j] = W;
+  }
+  recv_off[K] = k;
 }
 
 /* The rule of the header as first pinned: SGD (+ momentum), push-sum fold. */

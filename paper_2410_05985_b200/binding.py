@@ -27,19 +27,33 @@ class LayUpError(RuntimeError):
         self.code = code
 
 
+class _Tuning(ctypes.Structure):
+    """layup_tuning of include/layup.h: 0 = the library's default in every field."""
+    _fields_ = [(n, ctypes.c_int32) for n in ("engine", "launch_shape", "fused", "fused_waves", "tile_items", "variant",
+                                              "ctas_per_sm", "pdl", "tma2d", "stages")]
+
+
+ENGINE_TMA, ENGINE_LDG = 1, 2
+SHAPE_GROUPED, SHAPE_PERSISTENT = 1, 2
+FUSED_AUTO, FUSED_NEVER = 1, 2
+
+
 class _Config(ctypes.Structure):
     _fields_ = [("K", ctypes.c_int32), ("L", ctypes.c_int32), ("numel", ctypes.POINTER(ctypes.c_int64)),
                 ("lr", ctypes.c_float), ("momentum", ctypes.c_float), ("seed", ctypes.c_uint64),
                 ("peer_mode", ctypes.c_int32), ("skip_prob", ctypes.c_float), ("device", ctypes.c_int32),
                 ("delay_replica", ctypes.c_int32), ("delay_rounds", ctypes.c_int32),
                 ("optimizer", ctypes.c_int32), ("mix_mode", ctypes.c_int32), ("weight_decay", ctypes.c_float),
-                ("beta1", ctypes.c_float), ("beta2", ctypes.c_float), ("eps", ctypes.c_float)]
+                ("beta1", ctypes.c_float), ("beta2", ctypes.c_float), ("eps", ctypes.c_float),
+                ("tuning", ctypes.POINTER(_Tuning))]
 
 
 EXPORTS = ["layup_arena_bytes", "layup_init", "layup_destroy", "layup_ptr", "layup_set_lr",
            "layup_layer_update", "layup_round", "layup_round_host", "layup_sync", "layup_peer",
-           "layup_schedule", "layup_weights", "layup_state_export", "layup_state_import", "layup_disagreement", "layup_profile", "layup_profile_read", "layup_launch_count",
-           "layup_last_error"]
+           "layup_schedule", "layup_schedule_tables", "layup_last_order", "layup_trace", "layup_trace_read",
+           "layup_weights", "layup_state_export", "layup_state_import", "layup_disagreement", "layup_disagreement_ms",
+           "layup_graph_begin", "layup_graph_end", "layup_graph_launch", "layup_graph_destroy",
+           "layup_profile", "layup_profile_read", "layup_launch_count", "layup_last_error"]
 
 
 def load_library():
@@ -67,7 +81,16 @@ def load_library():
         "layup_weights": [vp, vp],
         "layup_state_export": [vp, vp, vp, vp],
         "layup_state_import": [vp, vp, vp, vp],
-        "layup_disagreement": [vp, i32, vp],
+        "layup_disagreement": [vp, i32, vp, vp],
+        "layup_disagreement_ms": [vp, c.POINTER(c.c_double)],
+        "layup_schedule_tables": [vp, i32, c.POINTER(i64), vp, vp, vp, vp, vp],
+        "layup_last_order": [vp, vp, c.POINTER(i32)],
+        "layup_trace": [vp, i32],
+        "layup_trace_read": [vp, vp],
+        "layup_graph_begin": [vp, vp],
+        "layup_graph_end": [vp, c.POINTER(vp)],
+        "layup_graph_launch": [vp, vp, vp],
+        "layup_graph_destroy": [vp, vp],
         "layup_profile": [vp, i32],
         "layup_profile_read": [vp, c.POINTER(i64), c.POINTER(c.c_double)],
         "layup_launch_count": [vp, c.POINTER(i64)],
@@ -86,12 +109,14 @@ def _check(rc, ctx=None):
 
 
 def _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device, delay_replica=0, delay_rounds=0,
-            optimizer=OPT_SGD, mix_mode=MIX_PUSHSUM, weight_decay=0.0, beta1=0.9, beta2=0.999, eps=1e-8):
+            optimizer=OPT_SGD, mix_mode=MIX_PUSHSUM, weight_decay=0.0, beta1=0.9, beta2=0.999, eps=1e-8, tuning=None):
     arr = (ctypes.c_int64 * len(numel))(*[int(n) for n in numel])
+    tune = _Tuning(**{k: int(v) for k, v in tuning.items()}) if tuning else None
     cfg = _Config(int(K), len(numel), arr, float(lr), float(momentum), int(seed), int(peer_mode),
                   float(skip_prob), int(device), int(delay_replica), int(delay_rounds),
-                  int(optimizer), int(mix_mode), float(weight_decay), float(beta1), float(beta2), float(eps))
-    cfg._keep = arr
+                  int(optimizer), int(mix_mode), float(weight_decay), float(beta1), float(beta2), float(eps),
+                  ctypes.pointer(tune) if tune is not None else None)
+    cfg._keep = (arr, tune)
     return cfg
 
 
@@ -128,14 +153,15 @@ class LayUp:
                  peer_mode: int = 0, skip_prob: float = 0.0, device: int = 0,
                  delay_replica: int = 0, delay_rounds: int = 0, optimizer: int = OPT_SGD,
                  mix_mode: int = MIX_PUSHSUM, weight_decay: float = 0.0, beta1: float = 0.9, beta2: float = 0.999,
-                 eps: float = 1e-8):
+                 eps: float = 1e-8, tuning: Optional[dict] = None):
+        """tuning: layup_tuning fields by name (include/layup.h), e.g. dict(launch_shape=SHAPE_PERSISTENT)."""
         self.lib = load_library()
         self.K, self.L, self.numel = int(K), len(numel), [int(n) for n in numel]
         self.momentum = float(momentum)
         self.device = torch.device("cuda", device)
         self.optimizer, self.mix_mode = int(optimizer), int(mix_mode)
         self._cfg = _config(K, numel, lr, momentum, seed, peer_mode, skip_prob, device, delay_replica, delay_rounds,
-                            optimizer, mix_mode, weight_decay, beta1, beta2, eps)
+                            optimizer, mix_mode, weight_decay, beta1, beta2, eps, tuning)
         nbytes = ctypes.c_size_t(0)
         _check(self.lib.layup_arena_bytes(ctypes.byref(self._cfg), ctypes.byref(nbytes)))
         self.arena_bytes = nbytes.value
@@ -191,6 +217,44 @@ class LayUp:
         _check(self.lib.layup_schedule(self.ctx, step, peer.ctypes.data, active.ctypes.data), self.ctx)
         return peer, active
 
+    def layup_schedule_tables(self, layer: int):
+        """-> dict(step, peer[K], flags[K], recv_off[K+1], senders[K], alpha[K]) as the update kernel consumed them."""
+        K = self.K
+        step = ctypes.c_int64()
+        peer, flags = np.empty(K, dtype=np.int32), np.empty(K, dtype=np.uint8)
+        recv_off, senders = np.empty(K + 1, dtype=np.int32), np.empty(K, dtype=np.int32)
+        alpha = np.empty(K, dtype=np.float32)
+        _check(self.lib.layup_schedule_tables(self.ctx, layer, ctypes.byref(step), peer.ctypes.data, flags.ctypes.data,
+                                              recv_off.ctypes.data, senders.ctypes.data, alpha.ctypes.data), self.ctx)
+        return dict(step=step.value, peer=peer, flags=flags, recv_off=recv_off, senders=senders, alpha=alpha)
+
+    def layup_last_order(self) -> List[int]:
+        out, n = np.empty(self.L, dtype=np.int32), ctypes.c_int32()
+        _check(self.lib.layup_last_order(self.ctx, out.ctypes.data, ctypes.byref(n)), self.ctx)
+        return [int(v) for v in out[:n.value]]
+
+    def layup_trace(self, enable: bool):
+        _check(self.lib.layup_trace(self.ctx, 1 if enable else 0), self.ctx)
+
+    def layup_trace_read(self) -> np.ndarray:
+        out = np.empty(self.L, dtype=np.uint64)
+        _check(self.lib.layup_trace_read(self.ctx, out.ctypes.data), self.ctx)
+        return out
+
+    def layup_graph_begin(self, stream):
+        _check(self.lib.layup_graph_begin(self.ctx, _stream_handle(stream, self.device.index)), self.ctx)
+
+    def layup_graph_end(self):
+        g = ctypes.c_void_p()
+        _check(self.lib.layup_graph_end(self.ctx, ctypes.byref(g)), self.ctx)
+        return g
+
+    def layup_graph_launch(self, graph, stream=None):
+        _check(self.lib.layup_graph_launch(self.ctx, graph, _stream_handle(stream, self.device.index)), self.ctx)
+
+    def layup_graph_destroy(self, graph):
+        _check(self.lib.layup_graph_destroy(self.ctx, graph), self.ctx)
+
     def layup_weights(self) -> np.ndarray:
         w = np.empty((self.L, self.K), dtype=np.float64)
         _check(self.lib.layup_weights(self.ctx, w.ctypes.data), self.ctx)
@@ -213,10 +277,16 @@ class LayUp:
         _check(self.lib.layup_state_import(self.ctx, w.ctypes.data, bp.ctypes.data if bp is not None else None,
                                            ns.ctypes.data), self.ctx)
 
-    def layup_disagreement(self, weighted: bool = False) -> np.ndarray:
+    def layup_disagreement(self, weighted: bool = False, stream=None) -> np.ndarray:
         d = np.empty((self.L, self.K), dtype=np.float64)
-        _check(self.lib.layup_disagreement(self.ctx, 1 if weighted else 0, d.ctypes.data), self.ctx)
+        _check(self.lib.layup_disagreement(self.ctx, 1 if weighted else 0, d.ctypes.data,
+                                           _stream_handle(stream, self.device.index)), self.ctx)
         return d
+
+    def layup_disagreement_ms(self) -> float:
+        ms = ctypes.c_double()
+        _check(self.lib.layup_disagreement_ms(self.ctx, ctypes.byref(ms)), self.ctx)
+        return ms.value
 
     def layup_profile(self, enable: bool):
         _check(self.lib.layup_profile(self.ctx, 1 if enable else 0), self.ctx)

@@ -31,11 +31,13 @@ struct layup_ctx {
   long long section = 0;                  // floats per section
   float *arena = nullptr;
   int C = 0, log2C = 0, smem = 0, ctas_per_sm = 1, n_sm = 1;
-  int variant = 0, threads = 256, launch_shape = -1;   // launch_shape: -1 auto, 0 grouped, 1 persistent
+  layup_tuning tune{};                                 // layup_config.tuning (zeros = defaults)
+  int variant = 0, threads = 256;
+  bool persistent = false;                             // tuning.launch_shape == 2
   int engine = 1;                                      // 1: TMA-staged kernel, 0: LDG kernel
   int32_t delay_replica = 0, delay_rounds = 0;
   int diag_C = 0, diag_log2C = 0, diag_smem = 0, diag_ctas = 1;
-  bool diag_two_stage = true;
+  int diag_stages = 0;
   double *d_dist = nullptr;
   // device tables
   LayerDesc *d_layers = nullptr;
@@ -44,13 +46,26 @@ struct layup_ctx {
   SchedTables t{};
   int32_t *d_peer_scratch = nullptr, *d_ticket = nullptr;
   void *d_tmaps = nullptr;                // [n_sections][L] CUtensorMap: 2-D tiled view [K][pad] of every layer section
-  bool ps_ok = false;                     // LAYUP_PERSISTENT=1: persistent two-stage form of the TMA kernel
-  int ps_smem = 0, ps_ctas = 0;
+  bool ps_ok = false;                     // tuning.launch_shape == 2: persistent form of the TMA kernel
+  int ps_smem = 0, ps_ctas = 0, ps_stages = 0;
   bool pdl = true;                        // programmatic dependent launch of the update kernel behind the schedule kernel
   bool fused_ok = false;                  // the single-launch path exists for this ctx (K, engine, variant)
   long long fused_max_tiles = 0;          // ... and is taken by launches of at most this many work items
   unsigned char *d_active_scratch = nullptr;
+  uint32_t *d_step = nullptr;             // [L] round each layer runs next (device state, see layup.h graphs)
+  unsigned long long *d_trace = nullptr;  // [L] layup_trace
+  bool tracing = false;
   // bookkeeping
+  bool poisoned = false;                  // a launching call failed half way (layup_round_host)
+  std::vector<int32_t> last_order;        // layup_last_order
+  std::vector<int64_t> last_event_step;   // [L] step of the most recent event of each layer (-1: none)
+  bool capturing = false;                 // between layup_graph_begin and layup_graph_end
+  cudaStream_t cap_stream = nullptr;
+  std::vector<int64_t> cap_next_step, cap_last_event;
+  std::vector<int32_t> cap_order;
+  int64_t cap_launches = 0;
+  cudaEvent_t diag_ev0 = nullptr, diag_ev1 = nullptr;
+  bool diag_timed = false;
   std::vector<cudaStream_t> streams;      // every stream launched on
   cudaStream_t own_stream = nullptr;      // introspection / init
   cudaStream_t s_h2d = nullptr, s_cmp = nullptr, s_d2h = nullptr;
@@ -61,7 +76,33 @@ struct layup_ctx {
   std::string err;
 };
 
+struct layup_graph {
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  layup_ctx *owner = nullptr;
+  std::vector<int64_t> advance;           // [L] rounds each layer moves per replay
+  std::vector<int32_t> order;             // layers in recorded issue order
+  int64_t launches = 0;                   // kernels per replay
+};
+
 static thread_local std::string g_err;
+
+// every entry point leaves the caller's current device as it found it
+struct DeviceGuard {
+  int prev = -1;
+  cudaError_t err;
+  explicit DeviceGuard(int dev) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev);
+  }
+  ~DeviceGuard() {
+    int cur = -1;
+    if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+  }
+};
+#define LAYUP_ON_DEVICE(ctx)       \
+  DeviceGuard guard__((ctx)->device); \
+  CU_TRY(ctx, guard__.err)
 
 static int fail(layup_ctx *ctx, int code, const char *fmt, ...) {
   char buf[512];
@@ -100,6 +141,13 @@ static int check_config(const layup_config *cfg) {
     return fail(nullptr, LAYUP_EINVAL, "AdamW needs 0 <= beta1, beta2 < 1 and eps >= 0");
   if (cfg->delay_rounds < 0 || (cfg->delay_rounds > 0 && (cfg->delay_replica < 0 || cfg->delay_replica >= cfg->K)))
     return fail(nullptr, LAYUP_EINVAL, "delay_replica / delay_rounds invalid");
+  if (cfg->tuning) {
+    const layup_tuning &t = *cfg->tuning;
+    if (t.engine < 0 || t.engine > 2 || t.launch_shape < 0 || t.launch_shape > 2 || t.fused < 0 || t.fused > 2 ||
+        t.pdl < 0 || t.pdl > 2 || t.tma2d < 0 || t.tma2d > 2 || t.fused_waves < 0 || t.tile_items < 0 ||
+        t.variant < 0 || t.ctas_per_sm < 0 || t.stages < 0)
+      return fail(nullptr, LAYUP_EINVAL, "layup_tuning field out of range");
+  }
   return LAYUP_OK;
 }
 
@@ -125,11 +173,6 @@ static void note_stream(layup_ctx *ctx, cudaStream_t s) {
   if (std::find(ctx->streams.begin(), ctx->streams.end(), s) == ctx->streams.end()) ctx->streams.push_back(s);
 }
 
-static int env_int(const char *name, int dflt) {
-  const char *v = getenv(name);
-  return v && *v ? atoi(v) : dflt;
-}
-
 extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena_bytes, layup_ctx **out) {
   int rc = check_config(cfg);
   if (rc) return rc;
@@ -143,9 +186,12 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   int ndev = 0;
   CU_TRY(nullptr, cudaGetDeviceCount(&ndev));
   if (cfg->device < 0 || cfg->device >= ndev) return fail(nullptr, LAYUP_EINVAL, "device %d of %d", cfg->device, ndev);
-  CU_TRY(nullptr, cudaSetDevice(cfg->device));
+  DeviceGuard guard(cfg->device);
+  CU_TRY(nullptr, guard.err);
 
   layup_ctx *ctx = new layup_ctx();
+  if (cfg->tuning) ctx->tune = *cfg->tuning;
+  const layup_tuning &tune = ctx->tune;
   ctx->K = cfg->K; ctx->L = cfg->L; ctx->device = cfg->device; ctx->peer_mode = cfg->peer_mode;
   ctx->lr = cfg->lr; ctx->mu = cfg->momentum; ctx->skip_prob = cfg->skip_prob; ctx->seed = cfg->seed;
   {
@@ -165,7 +211,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   // Measured on B200: ~1024 items per CTA (48 KB staged with momentum, 4 CTAs/SM) is
   // best while a replica's row of the tile is >= 1 KB; for K >= 32 rows of 1 KB (C = 64) beat more
   // CTAs per SM as long as two CTAs still fit (staged bytes <= 112 KB).
-  const int items_env = env_int("LAYUP_TILE_ITEMS", 0);
+  const int items_env = tune.tile_items;
   const int items_target = std::max(256, items_env > 0 ? items_env : 1024);
   int C = 8;
   while ((long long)cfg->K * C * 2 <= items_target && C < 4096) C *= 2;
@@ -209,14 +255,14 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     fail(nullptr, LAYUP_EINVAL, "K=%d needs %d B of shared memory per CTA", K, ctx->smem);
     return bail(LAYUP_EINVAL);
   }
-  ctx->engine = env_int("LAYUP_ENGINE", 1);
-  ctx->variant = env_int("LAYUP_VARIANT", 0);
-  ctx->launch_shape = env_int("LAYUP_PERSISTENT", -1);
-  ctx->pdl = env_int("LAYUP_PDL", 1) != 0;
+  ctx->engine = tune.engine == 2 ? 0 : 1;
+  ctx->variant = tune.variant;
+  ctx->persistent = tune.launch_shape == 2;
+  ctx->pdl = tune.pdl != 2;
   if (ctx->engine == 1) {
     // TMA-staged kernel stages x, g (, m) of the whole tile: fall back to the LDG kernel if it does not fit
     if (ctx->variant < 0 || ctx->variant >= tma_num_variants()) ctx->variant = 0;
-    ctx->fused_ok = K <= kFusedMaxK && tma_has_fused(ctx->variant) && env_int("LAYUP_FUSED", 1) != 0;
+    ctx->fused_ok = K <= kFusedMaxK && tma_has_fused(ctx->variant) && tune.fused != 2;
     const size_t need_smem = tma_smem_bytes(K, C, ctx->opt, ctx->fused_ok);
     if (need_smem > prop.sharedMemPerBlockOptin) { ctx->engine = 0; ctx->fused_ok = false; }
     else ctx->smem = (int)need_smem;
@@ -233,9 +279,9 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   //  HBM-sized rounds -- the redundant schedule stage is only free while the launch is latency bound)
   //  (K = 8 always fused: per-layer events 3.03 -> 2.97 ms per round, but AdamW rounds -0.7 % and
   //  straggler rounds -12 %, where the schedule stage sits in front of the loads: not done.)
-  const int waves = env_int("LAYUP_FUSED_WAVES", 4);
+  const int waves = tune.fused_waves > 0 ? tune.fused_waves : 4;
   ctx->fused_max_tiles = (long long)waves * ctx->n_sm * ctx->ctas_per_sm;
-  const int cap = env_int("LAYUP_CTAS_PER_SM", 0);
+  const int cap = tune.ctas_per_sm;
   if (cap > 0 && cap < ctx->ctas_per_sm) ctx->ctas_per_sm = cap;
 
   CU_TRY_INIT(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
@@ -261,10 +307,15 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   CU_TRY_INIT(cudaMemset(ctx->d_ticket, 0, sizeof(int32_t) * L));
   CU_TRY_INIT(cudaMalloc(&ctx->d_active_scratch, (size_t)K));
   CU_TRY_INIT(cudaMalloc(&ctx->d_dist, sizeof(double) * L * K));
+  CU_TRY_INIT(cudaMalloc(&ctx->d_step, sizeof(uint32_t) * L));
+  CU_TRY_INIT(cudaMemset(ctx->d_step, 0, sizeof(uint32_t) * L));
+  CU_TRY_INIT(cudaMalloc(&ctx->d_trace, sizeof(unsigned long long) * L));
+  CU_TRY_INIT(cudaMemset(ctx->d_trace, 0xFF, sizeof(unsigned long long) * L));
+  ctx->last_event_step.assign(L, -1);
   // 2-D tile loads replace K*arrays 1-D bulk copies per CTA by one per array.  Measured on B200: a
   // clear win without momentum (K = 16: 6.27 -> 6.94 TB/s) and from 64 copies per CTA up; at
   // K = 16 with momentum (48 copies) the 1-D form is 0.2 % ahead, so it is kept there.
-  const bool want_2d = env_int("LAYUP_TMA2D", (ctx->n_sections == 2 || K * ctx->n_sections >= 64) ? 1 : 0) != 0;
+  const bool want_2d = tune.tma2d == 1 || (tune.tma2d == 0 && (ctx->n_sections == 2 || K * ctx->n_sections >= 64));
   if (ctx->engine == 1 && want_2d && K <= 256 && C * 4 <= 256) {
     // One tensor map per (section, layer): rank 2, inner dim = the padded slice, outer dim = the K
     // replicas (stride = pad), box = [K][C*4 floats], no swizzle, zero fill past the slice end.
@@ -295,15 +346,26 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
       CU_TRY_INIT(cudaMemcpy(ctx->d_tmaps, maps.data(), sizeof(CUtensorMap) * maps.size(), cudaMemcpyHostToDevice));
     }
   }
-  if (ctx->engine == 1 && ctx->launch_shape == 1 && ctx->mix_mode != kMixSymmetric && ctx->skip_thr == 0u &&
-      ctx->delay_rounds == 0) {
-    ctx->ps_smem = (int)persist_smem_bytes(K, C, ctx->opt);
-    if ((size_t)ctx->ps_smem <= prop.sharedMemPerBlockOptin) {
-      CU_TRY_INIT(persist_kernel_setup(ctx->opt, ctx->ps_smem, &ctx->ps_ctas));
-      const int cap_ps = env_int("LAYUP_CTAS_PER_SM", 0);
-      if (cap_ps > 0 && cap_ps < ctx->ps_ctas) ctx->ps_ctas = cap_ps;
-      ctx->ps_ok = ctx->ps_ctas >= 1;
+  if (ctx->engine == 1 && ctx->persistent) {
+    // no silent fallback: the persistent shape either exists for this ctx or init says why not
+    if (K > persist_max_k()) {
+      fail(nullptr, LAYUP_EINVAL, "launch_shape = persistent needs K <= %d with the TMA engine", persist_max_k());
+      return bail(LAYUP_EINVAL);
     }
+    const int want_ctas = tune.ctas_per_sm > 0 ? tune.ctas_per_sm : 1;
+    ctx->ps_stages = persist_stages(K, C, ctx->opt, prop.sharedMemPerBlockOptin, want_ctas, tune.stages);
+    if (ctx->ps_stages < 2) {
+      fail(nullptr, LAYUP_EINVAL, "launch_shape = persistent: two stages of this tile do not fit in shared memory");
+      return bail(LAYUP_EINVAL);
+    }
+    ctx->ps_smem = (int)persist_smem_bytes(K, C, ctx->opt, ctx->ps_stages);
+    CU_TRY_INIT(persist_kernel_setup(ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->ps_smem, &ctx->ps_ctas));
+    if (ctx->ps_ctas > want_ctas) ctx->ps_ctas = want_ctas;
+    if (ctx->ps_ctas < 1) {
+      fail(nullptr, LAYUP_EINVAL, "launch_shape = persistent: the kernel does not fit on an SM");
+      return bail(LAYUP_EINVAL);
+    }
+    ctx->ps_ok = true;
   }
   CU_TRY_INIT(cudaMemcpy(ctx->d_layers, ctx->layers.data(), sizeof(LayerDesc) * L, cudaMemcpyHostToDevice));
   CU_TRY_INIT(cudaMemcpy(ctx->d_tile_prefix, ctx->tile_prefix.data(), sizeof(long long) * (L + 1), cudaMemcpyHostToDevice));
@@ -311,6 +373,9 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   CU_TRY_INIT(cudaMemcpy(ctx->d_w, w0.data(), sizeof(double) * L * K, cudaMemcpyHostToDevice));
   CU_TRY_INIT(cudaMemset(ctx->t.recv_off, 0, sizeof(int32_t) * L * (K + 1)));
   CU_TRY_INIT(cudaMemset(ctx->t.flags, 0, (size_t)L * K));
+  CU_TRY_INIT(cudaMemset(ctx->t.peer, 0xFF, sizeof(int32_t) * L * K));
+  CU_TRY_INIT(cudaMemset(ctx->t.senders, 0, sizeof(int32_t) * L * K));
+  CU_TRY_INIT(cudaMemset(ctx->t.alpha, 0, sizeof(float) * L * K));
   CU_TRY_INIT(cudaMemset(arena_dev, 0, need));                          // pads are zero and stay zero
   CU_TRY_INIT(cudaDeviceSynchronize());
 #undef CU_TRY_INIT
@@ -320,7 +385,13 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
 
 extern "C" int layup_destroy(layup_ctx *ctx) {
   if (!ctx) return LAYUP_OK;
-  cudaSetDevice(ctx->device);
+  DeviceGuard guard(ctx->device);
+  if (ctx->capturing) {                                    // abandon an open capture
+    cudaGraph_t g = nullptr;
+    cudaStreamEndCapture(ctx->cap_stream, &g);
+    if (g) cudaGraphDestroy(g);
+    cudaGetLastError();
+  }
   for (cudaStream_t s : ctx->streams) cudaStreamSynchronize(s);
   for (cudaStream_t s : {ctx->own_stream, ctx->s_h2d, ctx->s_cmp, ctx->s_d2h})
     if (s) { cudaStreamSynchronize(s); cudaStreamDestroy(s); }
@@ -328,10 +399,13 @@ extern "C" int layup_destroy(layup_ctx *ctx) {
     for (cudaEvent_t e : v) cudaEventDestroy(e);
   for (auto &pr : ctx->prof_pending) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
   for (auto &pr : ctx->prof_pool) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+  if (ctx->diag_ev0) cudaEventDestroy(ctx->diag_ev0);
+  if (ctx->diag_ev1) cudaEventDestroy(ctx->diag_ev1);
   cudaFree(ctx->d_layers); cudaFree(ctx->d_tile_prefix); cudaFree(ctx->d_w);
   cudaFree(ctx->t.peer); cudaFree(ctx->t.recv_off); cudaFree(ctx->t.senders); cudaFree(ctx->t.alpha);
   cudaFree(ctx->t.c1); cudaFree(ctx->t.c2); cudaFree(ctx->d_bpow);
-  cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_ticket); cudaFree(ctx->d_tmaps); cudaFree(ctx->d_active_scratch); cudaFree(ctx->d_dist);
+  cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_ticket); cudaFree(ctx->d_tmaps);
+  cudaFree(ctx->d_active_scratch); cudaFree(ctx->d_dist); cudaFree(ctx->d_step); cudaFree(ctx->d_trace);
   delete ctx;
   return LAYUP_OK;
 }
@@ -352,11 +426,21 @@ extern "C" int layup_set_lr(layup_ctx *ctx, float lr) {
   return LAYUP_OK;
 }
 
-// schedule kernel + update kernel for positions [pos_begin, pos_end) of the reverse-ordered list
-static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaStream_t s) {
+// what every launching call checks first
+static int check_launchable(layup_ctx *ctx, int64_t step, cudaStream_t s) {
+  if (ctx->poisoned) return fail(ctx, LAYUP_ECUDA, "ctx is poisoned: an earlier launching call failed half way through a round");
+  if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
+  if (ctx->capturing && s != ctx->cap_stream)
+    return fail(ctx, LAYUP_EINVAL, "a graph capture is open on another stream (layup_graph_begin)");
+  return LAYUP_OK;
+}
+
+// schedule kernel + update kernel for positions [pos_begin, pos_end) of the reverse-ordered list.
+// The round number itself is device state (d_step); `step` only feeds the host's bookkeeping.
+static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_t s, int *n_kernels) {
   const int L = ctx->L;
   SchedParams sp{};
-  sp.t = ctx->t; sp.w = ctx->d_w; sp.seed = ctx->seed; sp.step = (uint32_t)step; sp.skip_thr = ctx->skip_thr;
+  sp.t = ctx->t; sp.w = ctx->d_w; sp.seed = ctx->seed; sp.step_dev = ctx->d_step; sp.skip_thr = ctx->skip_thr;
   sp.K = ctx->K; sp.L = L; sp.peer_mode = ctx->peer_mode;
   sp.delay_replica = ctx->delay_replica; sp.delay_rounds = ctx->delay_rounds;
   sp.layer_begin = L - pos_end;                       // layers [L-pos_end, L-pos_begin)
@@ -364,14 +448,6 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   sp.lr = (double)ctx->lr; sp.beta1 = (double)ctx->beta1; sp.beta2 = (double)ctx->beta2;
   sp.ticket = ctx->d_ticket;
   const bool fused = ctx->fused_ok && ctx->tile_prefix[pos_end] - ctx->tile_prefix[pos_begin] <= ctx->fused_max_tiles;
-  // profiling brackets the whole issue: the schedule kernel (a few us, overlapped with the update
-  // kernel's prologue by the programmatic dependent launch) and the update kernel(s)
-  std::pair<cudaEvent_t, cudaEvent_t> ev{nullptr, nullptr};
-  if (ctx->profiling) {
-    if (!ctx->prof_pool.empty()) { ev = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
-    else { CU_TRY(ctx, cudaEventCreate(&ev.first)); CU_TRY(ctx, cudaEventCreate(&ev.second)); }
-    CU_TRY(ctx, cudaEventRecord(ev.first, s));
-  }
   if (!fused) CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
 
   UpdateParams up{};
@@ -390,12 +466,13 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   up.all_active = (ctx->skip_thr == 0u && ctx->delay_rounds == 0) ? 1 : 0;
   up.sched = sp;
   up.tmaps = ctx->d_tmaps;
+  up.trace = ctx->tracing ? ctx->d_trace : nullptr;
   const long long tiles = up.tile_end - up.tile_begin;
   const long long resident = (long long)ctx->n_sm * ctx->ctas_per_sm;
 
   int n_launch = 0;
   if (ctx->engine == 1) {
-    // grouped launch(es): one CTA per work item; the work-list table travels in the kernel parameters
+    // one launch per <= kMaxPos positions: the work-list table travels in the kernel parameters
     for (int q0 = pos_begin; q0 < pos_end;) {
       PosTable tab;
       int n = 0;
@@ -412,7 +489,7 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
       // only the first update launch directly follows the schedule kernel on the stream
       if (ctx->ps_ok && !fused) {
         const int grid = (int)std::min<long long>(tab.prefix[n], (long long)ctx->n_sm * ctx->ps_ctas);
-        CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->pdl && n_launch == 0, s));
+        CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->ps_stages, ctx->pdl && n_launch == 0, s));
       } else {
         CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, fused, ctx->pdl && n_launch == 0, (int)tab.prefix[n], ctx->smem, s));
       }
@@ -421,16 +498,41 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
     }
   } else {
     // LDG kernel: grouped (one CTA per work item) unless a persistent grid was asked for
-    const bool persistent = ctx->launch_shape == 1 || tiles > 0x7FFFFFFFll;
+    const bool persistent = ctx->persistent || tiles > 0x7FFFFFFFll;
     const int grid = (int)(persistent ? std::min<long long>(tiles, resident) : tiles);
     CU_TRY(ctx, launch_update(up, ctx->variant, persistent, grid, ctx->smem, s));
     n_launch = 1;
   }
-  if (ctx->profiling) {
-    CU_TRY(ctx, cudaEventRecord(ev.second, s));
-    ctx->prof_pending.push_back(ev);
+  *n_kernels = (fused ? 0 : 1) + n_launch;
+  return LAYUP_OK;
+}
+
+static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaStream_t s) {
+  // profiling brackets the whole issue: the schedule kernel (a few us, overlapped with the update
+  // kernel's prologue by the programmatic dependent launch) and the update kernel(s); not while
+  // a graph is being captured (nothing runs then)
+  std::pair<cudaEvent_t, cudaEvent_t> ev{nullptr, nullptr};
+  const bool prof = ctx->profiling && !ctx->capturing;
+  if (prof) {
+    if (!ctx->prof_pool.empty()) { ev = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
+    else {
+      CU_TRY(ctx, cudaEventCreate(&ev.first));
+      cudaError_t e = cudaEventCreate(&ev.second);
+      if (e != cudaSuccess) { cudaEventDestroy(ev.first); CU_TRY(ctx, e); }
+    }
   }
-  ctx->launches += (fused ? 0 : 1) + n_launch;
+  int n_kernels = 0;
+  int rc = LAYUP_OK;
+  if (prof && cudaEventRecord(ev.first, s) != cudaSuccess) rc = fail(ctx, LAYUP_ECUDA, "cudaEventRecord failed");
+  if (rc == LAYUP_OK) rc = issue_kernels(ctx, pos_begin, pos_end, s, &n_kernels);
+  if (rc == LAYUP_OK && prof && cudaEventRecord(ev.second, s) != cudaSuccess) rc = fail(ctx, LAYUP_ECUDA, "cudaEventRecord failed");
+  if (prof) (rc == LAYUP_OK ? ctx->prof_pending : ctx->prof_pool).push_back(ev);   // never leaked
+  if (rc != LAYUP_OK) return rc;
+  ctx->launches += n_kernels;
+  for (int p = pos_begin; p < pos_end; ++p) {
+    ctx->last_order.push_back(ctx->L - 1 - p);
+    ctx->last_event_step[ctx->L - 1 - p] = step;
+  }
   note_stream(ctx, s);
   return LAYUP_OK;
 }
@@ -438,24 +540,28 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
 extern "C" int layup_layer_update(layup_ctx *ctx, int64_t step, int32_t layer, void *cuda_stream) {
   if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
   if (layer < 0 || layer >= ctx->L) return fail(ctx, LAYUP_EINVAL, "layer %d out of range", layer);
-  if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
+  int rc = check_launchable(ctx, step, (cudaStream_t)cuda_stream);
+  if (rc) return rc;
   if (ctx->next_step[layer] != step)
     return fail(ctx, LAYUP_ESTATE, "layer %d expects step %lld, got %lld", layer, (long long)ctx->next_step[layer], (long long)step);
-  CU_TRY(ctx, cudaSetDevice(ctx->device));
+  LAYUP_ON_DEVICE(ctx);
   const int pos = ctx->L - 1 - layer;
-  int rc = issue(ctx, step, pos, pos + 1, (cudaStream_t)cuda_stream);
+  if (!ctx->capturing) ctx->last_order.clear();
+  rc = issue(ctx, step, pos, pos + 1, (cudaStream_t)cuda_stream);
   if (rc == LAYUP_OK) ctx->next_step[layer] = step + 1;
   return rc;
 }
 
 extern "C" int layup_round(layup_ctx *ctx, int64_t step, void *cuda_stream) {
   if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
-  if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
+  int rc = check_launchable(ctx, step, (cudaStream_t)cuda_stream);
+  if (rc) return rc;
   for (int l = 0; l < ctx->L; ++l)
     if (ctx->next_step[l] != step)
       return fail(ctx, LAYUP_ESTATE, "layer %d expects step %lld, got %lld", l, (long long)ctx->next_step[l], (long long)step);
-  CU_TRY(ctx, cudaSetDevice(ctx->device));
-  int rc = issue(ctx, step, 0, ctx->L, (cudaStream_t)cuda_stream);
+  LAYUP_ON_DEVICE(ctx);
+  if (!ctx->capturing) ctx->last_order.clear();
+  rc = issue(ctx, step, 0, ctx->L, (cudaStream_t)cuda_stream);
   if (rc == LAYUP_OK)
     for (int l = 0; l < ctx->L; ++l) ctx->next_step[l] = step + 1;
   return rc;
@@ -463,54 +569,87 @@ extern "C" int layup_round(layup_ctx *ctx, int64_t step, void *cuda_stream) {
 
 extern "C" int layup_round_host(layup_ctx *ctx, int64_t step, const float *g_host, float *x_host) {
   if (!ctx || !g_host) return fail(ctx, LAYUP_EINVAL, "ctx or g_host is NULL");
-  if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
+  if (ctx->capturing) return fail(ctx, LAYUP_ESTATE, "layup_round_host cannot be recorded into a graph");
+  int rc = check_launchable(ctx, step, nullptr);
+  if (rc) return rc;
   const int L = ctx->L, K = ctx->K;
   for (int l = 0; l < L; ++l)
     if (ctx->next_step[l] != step)
       return fail(ctx, LAYUP_ESTATE, "layer %d expects step %lld, got %lld", l, (long long)ctx->next_step[l], (long long)step);
-  CU_TRY(ctx, cudaSetDevice(ctx->device));
+  LAYUP_ON_DEVICE(ctx);
   if (!ctx->s_h2d) {
     CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->s_h2d, cudaStreamNonBlocking));
     CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->s_cmp, cudaStreamNonBlocking));
     CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->s_d2h, cudaStreamNonBlocking));
-    ctx->ev_h2d.resize(L); ctx->ev_done.resize(L);
-    for (int l = 0; l < L; ++l) {
-      CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->ev_h2d[l], cudaEventDisableTiming));
-      CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->ev_done[l], cudaEventDisableTiming));
+  }
+  if ((int)ctx->ev_done.size() < L) {
+    ctx->ev_h2d.reserve(L); ctx->ev_done.reserve(L);
+    while ((int)ctx->ev_h2d.size() < L) {
+      cudaEvent_t e;
+      CU_TRY(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+      ctx->ev_h2d.push_back(e);
+    }
+    while ((int)ctx->ev_done.size() < L) {
+      cudaEvent_t e;
+      CU_TRY(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+      ctx->ev_done.push_back(e);
     }
   }
   std::vector<long long> hoff(L + 1, 0);                   // host offsets, layer-major, unpadded
   for (int l = 0; l < L; ++l) hoff[l + 1] = hoff[l] + (long long)K * ctx->layers[l].numel;
   float *gsec = ctx->arena + ctx->section;
-  for (int l = L - 1; l >= 0; --l) {                       // output layer first
-    const LayerDesc &d = ctx->layers[l];
-    const size_t row = (size_t)d.numel * sizeof(float);
-    CU_TRY(ctx, cudaMemcpy2DAsync(gsec + d.base, (size_t)d.pad * sizeof(float), g_host + hoff[l], row, row, K,
-                                  cudaMemcpyHostToDevice, ctx->s_h2d));
-    CU_TRY(ctx, cudaEventRecord(ctx->ev_h2d[l], ctx->s_h2d));
-    CU_TRY(ctx, cudaStreamWaitEvent(ctx->s_cmp, ctx->ev_h2d[l], 0));
-    const int pos = L - 1 - l;
-    int rc = issue(ctx, step, pos, pos + 1, ctx->s_cmp);
-    if (rc) return rc;
-    ctx->next_step[l] = step + 1;
-    if (x_host) {
-      CU_TRY(ctx, cudaEventRecord(ctx->ev_done[l], ctx->s_cmp));
-      CU_TRY(ctx, cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_done[l], 0));
-      CU_TRY(ctx, cudaMemcpy2DAsync(x_host + hoff[l], row, ctx->arena + d.base, (size_t)d.pad * sizeof(float), row, K,
-                                    cudaMemcpyDeviceToHost, ctx->s_d2h));
+  ctx->last_order.clear();
+  // validate-then-commit: next_step moves only after the whole round is on the device and done
+  auto pipeline = [&]() -> int {
+    for (int l = L - 1; l >= 0; --l) {                     // output layer first
+      const LayerDesc &d = ctx->layers[l];
+      const size_t row = (size_t)d.numel * sizeof(float);
+      CU_TRY(ctx, cudaMemcpy2DAsync(gsec + d.base, (size_t)d.pad * sizeof(float), g_host + hoff[l], row, row, K,
+                                    cudaMemcpyHostToDevice, ctx->s_h2d));
+      CU_TRY(ctx, cudaEventRecord(ctx->ev_h2d[l], ctx->s_h2d));
+      CU_TRY(ctx, cudaStreamWaitEvent(ctx->s_cmp, ctx->ev_h2d[l], 0));
+      const int pos = L - 1 - l;
+      int r = issue(ctx, step, pos, pos + 1, ctx->s_cmp);
+      if (r) return r;
+      if (x_host) {
+        CU_TRY(ctx, cudaEventRecord(ctx->ev_done[l], ctx->s_cmp));
+        CU_TRY(ctx, cudaStreamWaitEvent(ctx->s_d2h, ctx->ev_done[l], 0));
+        CU_TRY(ctx, cudaMemcpy2DAsync(x_host + hoff[l], row, ctx->arena + d.base, (size_t)d.pad * sizeof(float), row, K,
+                                      cudaMemcpyDeviceToHost, ctx->s_d2h));
+      }
     }
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->s_h2d));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->s_cmp));
+    CU_TRY(ctx, cudaStreamSynchronize(ctx->s_d2h));
+    return LAYUP_OK;
+  };
+  rc = pipeline();
+  if (rc != LAYUP_OK) {
+    // the host buffers must not be in use when we return; the arena holds a partial round
+    const std::string why = ctx->err;
+    cudaStreamSynchronize(ctx->s_h2d);
+    cudaStreamSynchronize(ctx->s_cmp);
+    cudaStreamSynchronize(ctx->s_d2h);
+    cudaGetLastError();
+    ctx->poisoned = true;
+    return fail(ctx, LAYUP_ECUDA, "layup_round_host failed mid-round, ctx poisoned: %s", why.c_str());
   }
-  CU_TRY(ctx, cudaStreamSynchronize(ctx->s_h2d));
-  CU_TRY(ctx, cudaStreamSynchronize(ctx->s_cmp));
-  CU_TRY(ctx, cudaStreamSynchronize(ctx->s_d2h));
+  for (int l = 0; l < L; ++l) ctx->next_step[l] = step + 1;
   return LAYUP_OK;
 }
 
 extern "C" int layup_sync(layup_ctx *ctx) {
   if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
-  CU_TRY(ctx, cudaSetDevice(ctx->device));
+  if (ctx->capturing) return fail(ctx, LAYUP_ESTATE, "a graph capture is open (layup_graph_end first)");
+  LAYUP_ON_DEVICE(ctx);
   for (cudaStream_t s : ctx->streams) CU_TRY(ctx, cudaStreamSynchronize(s));
   CU_TRY(ctx, cudaGetLastError());
+  // the device's round counters against the host's bookkeeping (graphs replay on the device's word)
+  std::vector<uint32_t> dev(ctx->L);
+  CU_TRY(ctx, cudaMemcpy(dev.data(), ctx->d_step, sizeof(uint32_t) * ctx->L, cudaMemcpyDeviceToHost));
+  for (int l = 0; l < ctx->L; ++l)
+    if (dev[l] != (uint32_t)ctx->next_step[l])
+      return fail(ctx, LAYUP_ESTATE, "layer %d: device ran %u rounds, host expected %lld", l, dev[l], (long long)ctx->next_step[l]);
   return LAYUP_OK;
 }
 
@@ -522,8 +661,9 @@ extern "C" int layup_peer(uint64_t seed, int64_t step, int32_t layer, int32_t re
 
 extern "C" int layup_schedule(layup_ctx *ctx, int64_t step, int32_t *peer, uint8_t *active) {
   if (!ctx || !peer || !active) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  if (ctx->capturing) return fail(ctx, LAYUP_ESTATE, "a graph capture is open");
   if (step < 0 || step > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "step %lld outside [0, 2^32)", (long long)step);
-  CU_TRY(ctx, cudaSetDevice(ctx->device));
+  LAYUP_ON_DEVICE(ctx);
   CU_TRY(ctx, launch_peers_only(ctx->seed, (uint32_t)step, ctx->skip_thr, ctx->K, ctx->L, ctx->peer_mode,
                                 ctx->delay_replica, ctx->delay_rounds, ctx->d_peer_scratch, ctx->d_active_scratch, ctx->own_stream));
   ctx->launches += 1;
@@ -533,10 +673,56 @@ extern "C" int layup_schedule(layup_ctx *ctx, int64_t step, int32_t *peer, uint8
   return LAYUP_OK;
 }
 
+extern "C" int layup_schedule_tables(layup_ctx *ctx, int32_t layer, int64_t *step_done, int32_t *peer, uint8_t *flags,
+                                     int32_t *recv_off, int32_t *senders, float *alpha) {
+  if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
+  if (layer < 0 || layer >= ctx->L) return fail(ctx, LAYUP_EINVAL, "layer %d out of range", layer);
+  int rc = layup_sync(ctx);
+  if (rc) return rc;
+  LAYUP_ON_DEVICE(ctx);
+  const int K = ctx->K;
+  const size_t row = (size_t)layer * K;
+  if (step_done) *step_done = ctx->last_event_step[layer];
+  if (peer) CU_TRY(ctx, cudaMemcpy(peer, ctx->t.peer + row, sizeof(int32_t) * K, cudaMemcpyDeviceToHost));
+  if (flags) CU_TRY(ctx, cudaMemcpy(flags, ctx->t.flags + row, (size_t)K, cudaMemcpyDeviceToHost));
+  if (recv_off) CU_TRY(ctx, cudaMemcpy(recv_off, ctx->t.recv_off + (size_t)layer * (K + 1), sizeof(int32_t) * (K + 1), cudaMemcpyDeviceToHost));
+  if (senders) CU_TRY(ctx, cudaMemcpy(senders, ctx->t.senders + row, sizeof(int32_t) * K, cudaMemcpyDeviceToHost));
+  if (alpha) CU_TRY(ctx, cudaMemcpy(alpha, ctx->t.alpha + row, sizeof(float) * K, cudaMemcpyDeviceToHost));
+  return LAYUP_OK;
+}
+
+extern "C" int layup_last_order(layup_ctx *ctx, int32_t *layers, int32_t *n) {
+  if (!ctx || !layers || !n) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  const size_t m = std::min(ctx->last_order.size(), (size_t)ctx->L);
+  for (size_t k = 0; k < m; ++k) layers[k] = ctx->last_order[k];
+  *n = (int32_t)m;
+  return LAYUP_OK;
+}
+
+extern "C" int layup_trace(layup_ctx *ctx, int32_t enable) {
+  if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
+  int rc = layup_sync(ctx);
+  if (rc) return rc;
+  LAYUP_ON_DEVICE(ctx);
+  ctx->tracing = enable != 0;
+  if (ctx->tracing) CU_TRY(ctx, cudaMemset(ctx->d_trace, 0xFF, sizeof(unsigned long long) * ctx->L));
+  return LAYUP_OK;
+}
+
+extern "C" int layup_trace_read(layup_ctx *ctx, uint64_t *first_ns) {
+  if (!ctx || !first_ns) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  int rc = layup_sync(ctx);
+  if (rc) return rc;
+  LAYUP_ON_DEVICE(ctx);
+  CU_TRY(ctx, cudaMemcpy(first_ns, ctx->d_trace, sizeof(uint64_t) * ctx->L, cudaMemcpyDeviceToHost));
+  return LAYUP_OK;
+}
+
 extern "C" int layup_weights(layup_ctx *ctx, double *w) {
   if (!ctx || !w) return fail(ctx, LAYUP_EINVAL, "NULL argument");
   int rc = layup_sync(ctx);
   if (rc) return rc;
+  LAYUP_ON_DEVICE(ctx);
   CU_TRY(ctx, cudaMemcpy(w, ctx->d_w, sizeof(double) * ctx->L * ctx->K, cudaMemcpyDeviceToHost));
   return LAYUP_OK;
 }
@@ -546,6 +732,7 @@ extern "C" int layup_state_export(layup_ctx *ctx, double *w, double *bpow, int64
   if (ctx->opt == OPT_ADAMW && !bpow) return fail(ctx, LAYUP_EINVAL, "bpow is NULL but the optimizer is AdamW");
   int rc = layup_sync(ctx);
   if (rc) return rc;
+  LAYUP_ON_DEVICE(ctx);
   const size_t n = (size_t)ctx->L * ctx->K;
   CU_TRY(ctx, cudaMemcpy(w, ctx->d_w, sizeof(double) * n, cudaMemcpyDeviceToHost));
   if (ctx->opt == OPT_ADAMW) CU_TRY(ctx, cudaMemcpy(bpow, ctx->d_bpow, sizeof(double) * 2 * n, cudaMemcpyDeviceToHost));
@@ -560,33 +747,37 @@ extern "C" int layup_state_import(layup_ctx *ctx, const double *w, const double 
     if (next_step[l] < 0 || next_step[l] > 0xFFFFFFFFll) return fail(ctx, LAYUP_EINVAL, "next_step[%d] outside [0, 2^32)", l);
   int rc = layup_sync(ctx);
   if (rc) return rc;
+  LAYUP_ON_DEVICE(ctx);
   const size_t n = (size_t)ctx->L * ctx->K;
   CU_TRY(ctx, cudaMemcpy(ctx->d_w, w, sizeof(double) * n, cudaMemcpyHostToDevice));
   if (ctx->opt == OPT_ADAMW) CU_TRY(ctx, cudaMemcpy(ctx->d_bpow, bpow, sizeof(double) * 2 * n, cudaMemcpyHostToDevice));
-  for (int l = 0; l < ctx->L; ++l) ctx->next_step[l] = next_step[l];
+  std::vector<uint32_t> dev(ctx->L);
+  for (int l = 0; l < ctx->L; ++l) { ctx->next_step[l] = next_step[l]; dev[l] = (uint32_t)next_step[l]; }
+  CU_TRY(ctx, cudaMemcpy(ctx->d_step, dev.data(), sizeof(uint32_t) * ctx->L, cudaMemcpyHostToDevice));
   return LAYUP_OK;
 }
 
-extern "C" int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist) {
+extern "C" int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist, void *cuda_stream) {
   if (!ctx || !dist) return fail(ctx, LAYUP_EINVAL, "NULL argument");
-  int rc = layup_sync(ctx);
+  int rc = layup_sync(ctx);                       // everything this ctx issued, on whatever stream
   if (rc) return rc;
+  LAYUP_ON_DEVICE(ctx);
   const int K = ctx->K, L = ctx->L;
   if (ctx->diag_C == 0) {
-    // read-only tile: ~2048 float4 items (32 KB) of x per work item
-    int C = 8;
-    while ((long long)K * C * 2 <= 2048 && C < 256) C *= 2;       // C divides the 256 threads of the kernel
-    ctx->diag_C = C;
-    while ((1 << ctx->diag_log2C) < C) ++ctx->diag_log2C;
     cudaDeviceProp prop;
     CU_TRY(ctx, cudaGetDeviceProperties(&prop, ctx->device));
-    ctx->diag_two_stage = diag_smem_bytes(K, C, true) <= prop.sharedMemPerBlockOptin;   // else one stage (K > ~880)
-    ctx->diag_smem = (int)diag_smem_bytes(K, C, ctx->diag_two_stage);
-    CU_TRY(ctx, diag_setup(K, C, ctx->diag_smem, &ctx->diag_ctas));
-    if (ctx->diag_ctas < 1) return fail(ctx, LAYUP_EINVAL, "K=%d does not fit the diagnostic kernel", K);
+    rc = LAYUP_OK;
+    int C = 0, smem = 0, ctas = 0, stages = 0;
+    CU_TRY(ctx, diag_plan(K, (size_t)prop.sharedMemPerBlockOptin, &C, &stages, &smem, &ctas));
+    if (ctas < 1) return fail(ctx, LAYUP_EINVAL, "K=%d does not fit the diagnostic kernel", K);
+    ctx->diag_C = C; ctx->diag_smem = smem; ctx->diag_ctas = ctas; ctx->diag_stages = stages;
+    while ((1 << ctx->diag_log2C) < C) ++ctx->diag_log2C;
+    CU_TRY(ctx, cudaEventCreate(&ctx->diag_ev0));
+    CU_TRY(ctx, cudaEventCreate(&ctx->diag_ev1));
   }
-  cudaStream_t s = ctx->own_stream;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
   CU_TRY(ctx, cudaMemsetAsync(ctx->d_dist, 0, sizeof(double) * L * K, s));
+  CU_TRY(ctx, cudaEventRecord(ctx->diag_ev0, s));
   const int C = ctx->diag_C;
   for (int q0 = 0; q0 < L;) {
     PosTable tab;
@@ -603,12 +794,107 @@ extern "C" int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist
     const long long tiles = tab.prefix[n];
     const int grid = (int)std::min<long long>(tiles, (long long)ctx->n_sm * ctx->diag_ctas);
     CU_TRY(ctx, launch_disagreement(ctx->arena, weighted ? ctx->d_w : nullptr, ctx->d_dist, K, C, ctx->diag_log2C,
-                                    ctx->diag_two_stage, tab, grid, ctx->diag_smem, s));
+                                    ctx->diag_stages, tab, grid, ctx->diag_smem, s));
     ctx->launches += 1;
     q0 += n;
   }
+  CU_TRY(ctx, cudaEventRecord(ctx->diag_ev1, s));
   CU_TRY(ctx, cudaMemcpyAsync(dist, ctx->d_dist, sizeof(double) * L * K, cudaMemcpyDeviceToHost, s));
   CU_TRY(ctx, cudaStreamSynchronize(s));
+  ctx->diag_timed = true;
+  return LAYUP_OK;
+}
+
+extern "C" int layup_disagreement_ms(layup_ctx *ctx, double *ms) {
+  if (!ctx || !ms) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  if (!ctx->diag_timed) return fail(ctx, LAYUP_ESTATE, "layup_disagreement has not run yet");
+  LAYUP_ON_DEVICE(ctx);
+  float f = 0.f;
+  CU_TRY(ctx, cudaEventElapsedTime(&f, ctx->diag_ev0, ctx->diag_ev1));
+  *ms = f;
+  return LAYUP_OK;
+}
+
+// ---- CUDA-graph capture ---------------------------------------------------------------
+extern "C" int layup_graph_begin(layup_ctx *ctx, void *cuda_stream) {
+  if (!ctx) return fail(nullptr, LAYUP_EINVAL, "ctx is NULL");
+  if (!cuda_stream) return fail(ctx, LAYUP_EINVAL, "the legacy default stream cannot be captured");
+  if (ctx->capturing) return fail(ctx, LAYUP_ESTATE, "a graph capture is already open");
+  if (ctx->poisoned) return fail(ctx, LAYUP_ECUDA, "ctx is poisoned");
+  LAYUP_ON_DEVICE(ctx);
+  CU_TRY(ctx, cudaStreamBeginCapture((cudaStream_t)cuda_stream, cudaStreamCaptureModeRelaxed));
+  ctx->capturing = true;
+  ctx->cap_stream = (cudaStream_t)cuda_stream;
+  ctx->cap_next_step = ctx->next_step;           // nothing runs during capture: restored at the end
+  ctx->cap_last_event = ctx->last_event_step;
+  ctx->cap_order = ctx->last_order;
+  ctx->cap_launches = ctx->launches;
+  ctx->last_order.clear();
+  return LAYUP_OK;
+}
+
+extern "C" int layup_graph_end(layup_ctx *ctx, layup_graph **out) {
+  if (!ctx || !out) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  if (!ctx->capturing) return fail(ctx, LAYUP_ESTATE, "no graph capture is open");
+  LAYUP_ON_DEVICE(ctx);
+  *out = nullptr;
+  layup_graph *g = new layup_graph();
+  g->owner = ctx;
+  g->advance.resize(ctx->L);
+  for (int l = 0; l < ctx->L; ++l) g->advance[l] = ctx->next_step[l] - ctx->cap_next_step[l];
+  g->order = ctx->last_order;
+  g->launches = ctx->launches - ctx->cap_launches;
+  // roll the bookkeeping back: the recorded calls have not run
+  ctx->next_step = ctx->cap_next_step;
+  ctx->last_event_step = ctx->cap_last_event;
+  ctx->last_order = ctx->cap_order;
+  ctx->launches = ctx->cap_launches;
+  ctx->capturing = false;
+  cudaError_t e = cudaStreamEndCapture(ctx->cap_stream, &g->graph);
+  if (e == cudaSuccess && !g->graph) e = cudaErrorStreamCaptureInvalidated;
+  if (e == cudaSuccess) e = cudaGraphInstantiate(&g->exec, g->graph, 0);
+  if (e != cudaSuccess) {
+    if (g->graph) cudaGraphDestroy(g->graph);
+    delete g;
+    cudaGetLastError();
+    return fail(ctx, LAYUP_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
+  }
+  *out = g;
+  return LAYUP_OK;
+}
+
+extern "C" int layup_graph_launch(layup_ctx *ctx, layup_graph *g, void *cuda_stream) {
+  if (!ctx || !g) return fail(ctx, LAYUP_EINVAL, "NULL argument");
+  if (g->owner != ctx) return fail(ctx, LAYUP_EINVAL, "graph belongs to another ctx");
+  if (ctx->capturing) return fail(ctx, LAYUP_ESTATE, "a graph capture is open");
+  if (ctx->poisoned) return fail(ctx, LAYUP_ECUDA, "ctx is poisoned");
+  for (int l = 0; l < ctx->L; ++l)
+    if (ctx->next_step[l] + g->advance[l] > 0x100000000ll) return fail(ctx, LAYUP_EINVAL, "layer %d would pass step 2^32", l);
+  LAYUP_ON_DEVICE(ctx);
+  CU_TRY(ctx, cudaGraphLaunch(g->exec, (cudaStream_t)cuda_stream));
+  for (int l = 0; l < ctx->L; ++l) {
+    if (g->advance[l] > 0) ctx->last_event_step[l] = ctx->next_step[l] + g->advance[l] - 1;
+    ctx->next_step[l] += g->advance[l];
+  }
+  ctx->last_order = g->order;
+  ctx->launches += g->launches;
+  note_stream(ctx, (cudaStream_t)cuda_stream);
+  return LAYUP_OK;
+}
+
+extern "C" int layup_graph_destroy(layup_ctx *ctx, layup_graph *g) {
+  if (!g) return LAYUP_OK;
+  if (ctx && g->owner != ctx) return fail(ctx, LAYUP_EINVAL, "graph belongs to another ctx");
+  if (ctx) {
+    DeviceGuard guard(ctx->device);
+    for (cudaStream_t s : ctx->streams) cudaStreamSynchronize(s);
+    cudaGraphExecDestroy(g->exec);
+    cudaGraphDestroy(g->graph);
+  } else {
+    cudaGraphExecDestroy(g->exec);
+    cudaGraphDestroy(g->graph);
+  }
+  delete g;
   return LAYUP_OK;
 }
 
@@ -622,6 +908,7 @@ extern "C" int layup_profile_read(layup_ctx *ctx, int64_t *launches, double *tot
   if (!ctx || !launches || !total_ms) return fail(ctx, LAYUP_EINVAL, "NULL argument");
   int rc = layup_sync(ctx);
   if (rc) return rc;
+  LAYUP_ON_DEVICE(ctx);
   double tot = 0.0;
   for (auto &pr : ctx->prof_pending) {
     float ms = 0.f;

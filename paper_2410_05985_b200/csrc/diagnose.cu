@@ -3,14 +3,23 @@
 // (the paper's plain average) or c_i = w_i (push-sum weighted consensus).
 // PAPER.md:389-395 (Fig. A1 "model disagreement between workers"), eq. (9) PAPER.md:551.
 //
-// The only place on the path that needs norms, hence the only warp-level reductions.  Same tiling
-// as the update kernel -- a CTA owns a tile of C float4 columns for ALL K replicas, staged by TMA
-// bulk copies -- but read-only: 4 B of HBM traffic per parameter.  A persistent grid walks the
-// work list with a static stride through a two-stage shared-memory pipeline (the next tile is in
-// flight while this one is reduced).  A thread meets the same (replica, column) slots in every
-// tile, so it keeps its partial sums in registers and the cross-thread reduction (warp shuffles,
-// then one shared and one global fp64 atomic per replica) happens once per layer and CTA, not once
-// per tile.  Everything is accumulated in fp64 (sums are order-dependent in the last bits).
+// The only place on the path that needs norms, hence the only warp-level reductions.  Read-only:
+// 4 B of HBM traffic per parameter, so the roofline is the HBM read rate.
+//
+// Ring kernel (K <= 64), warp specialised:
+//   * one PRODUCER warp per CTA streams tiles (all K replicas x TF floats) into an S-stage shared
+//     memory ring with 1-D TMA bulk copies (cp.async.bulk, SASS UBLKCP), one copy per replica row
+//     spread over the warp's lanes, completing on the stage's "full" mbarrier; it re-arms a stage
+//     as soon as the stage's "empty" mbarrier has seen every consumer warp;
+//   * the CONSUMER warps never meet a CTA-wide barrier: a thread owns VEC scalar columns of the
+//     tile for ALL K replicas, so the consensus of its columns and the K squared distances are
+//     register arithmetic (fp64), with no exchange through shared memory.  For K <= 16 every
+//     element is converted to fp64 once and kept in registers for both passes, and the stage is
+//     released right after the loads; for larger K the second pass re-reads shared memory;
+//   * a CTA walks a CONTIGUOUS range of the tile list, so it crosses a layer boundary only a few
+//     times; the per-replica partial sums stay in registers until then and leave through warp
+//     shuffles and one fp64 atomicAdd per (warp, replica).
+// General kernel (K > 64): the earlier one-stage form, consensus through shared memory.
 #include "layup_internal.cuh"
 #include "tma_ptx.cuh"
 
@@ -18,28 +27,199 @@ namespace layup {
 
 namespace {
 
-constexpr int kDiagThreads = 256;
+constexpr int kConsumers = 256;                 // consumer threads per CTA (8 warps)
+constexpr int kRingThreads = kConsumers + 32;   // + the producer warp
 
 struct DiagParams {
   const float *x;          // X section base
   const double *w;         // [L*K] push-sum weights, or nullptr for the plain mean
   double *dist;            // [L*K] output, zeroed before the launch
-  int32_t K, C, log2C;
-  int32_t two_stage;       // 1: prefetch the next tile into a second stage; 0: one stage (very large K)
+  int32_t K, C, log2C;     // C = float4 columns per tile
+  int32_t stages;          // ring depth (ring kernel); 1 or 2 (general kernel)
 };
 
-// MAXIT >= ceil(K*C / kDiagThreads): register accumulators per thread
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+  return v;
+}
+
+// KT: compile-time bound on K (loops fully unrolled, accumulators in registers)
+// VEC: scalar columns per thread (tile row = kConsumers * VEC floats)
+// KEEP: keep the converted tile in registers between the two passes (one fp32->fp64 conversion per element)
+template <int KT, int VEC, bool KEEP, int MINB>
+__global__ void __launch_bounds__(kRingThreads, MINB)
+    layup_disagreement_kernel(const __grid_constant__ DiagParams p, const __grid_constant__ PosTable tab) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int TF = kConsumers * VEC;                                   // floats per replica row of a tile
+  const int K = p.K, S = p.stages, tid = threadIdx.x;
+  float *ring = reinterpret_cast<float *>(smem_raw);                    // [S][K][TF]
+  uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)S * K * TF);   // [S]
+  uint64_t *empty = full + S;                                           // [S]
+  double *coef_all = reinterpret_cast<double *>(empty + S);             // [consumer warps][KT] weighted mode only
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) {
+      mbar_init(full + s, 1);
+      mbar_init(empty + s, kConsumers / 32);
+    }
+  }
+  __syncthreads();
+
+  // contiguous share of the tile list
+  const long long n_tiles = tab.prefix[tab.n];
+  const long long t0 = n_tiles * blockIdx.x / gridDim.x, t1 = n_tiles * (blockIdx.x + 1) / gridDim.x;
+  if (t0 >= t1) return;
+  int pos = 0;
+  {
+    int lo = 0, hi = tab.n;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (t0 >= tab.prefix[mid]) lo = mid; else hi = mid;
+    }
+    pos = lo;
+  }
+
+  if (tid >= kConsumers) {
+    // ---------------- producer warp
+    const int lane = tid - kConsumers;
+    int s = 0;
+    uint32_t ph = 0;
+    for (long long tile = t0; tile < t1; ++tile) {
+      while (tile >= tab.prefix[pos + 1]) ++pos;
+      const long long pad = tab.lay[pos].pad;
+      const long long f0 = (tile - tab.prefix[pos]) * TF;               // first float of the tile in a slice
+      const long long left = pad - f0;
+      const uint32_t chunk = (uint32_t)(left < TF ? left : TF) * 4u;     // multiple of 128 B
+      const float *src = p.x + tab.lay[pos].base + f0;
+      mbar_wait(empty + s, ph ^ 1u);                                    // the first pass over the ring is free
+      if (lane == 0) mbar_expect_tx(full + s, chunk * (uint32_t)K);
+      __syncwarp();
+      float *dst = ring + (size_t)s * K * TF;
+      for (int i = lane; i < K; i += 32) bulk_g2s(dst + (size_t)i * TF, src + (long long)i * pad, chunk, full + s);
+      if (++s == S) { s = 0; ph ^= 1u; }
+    }
+    return;
+  }
+
+  // ---------------- consumers: thread owns columns [VEC*tid, VEC*tid + VEC) for all K replicas
+  // consensus coefficients: the scalar 1/K, or this layer's push-sum weights in a per-warp copy
+  // (warps cross layer boundaries at different times and never synchronise with each other)
+  double acc[KT];
+#pragma unroll
+  for (int i = 0; i < KT; ++i) acc[i] = 0.0;
+  const double inv_k = 1.0 / (double)K;
+  double *coef = coef_all + (size_t)(tid >> 5) * KT;
+  const bool weighted = p.w != nullptr;
+  auto load_coef = [&](int q) {
+    if (!weighted) return;
+    __syncwarp();
+    for (int i = tid & 31; i < K; i += 32) coef[i] = __ldg(p.w + (size_t)tab.layer[q] * K + i);
+    __syncwarp();
+  };
+  auto flush = [&](int q) {
+#pragma unroll
+    for (int i = 0; i < KT; ++i) {
+      if (i < K) {
+        const double v = warp_sum(acc[i]);
+        if ((tid & 31) == 0) atomicAdd(p.dist + (size_t)tab.layer[q] * K + i, v);
+      }
+      acc[i] = 0.0;
+    }
+  };
+  load_coef(pos);
+  int s = 0;
+  uint32_t ph = 0;
+  for (long long tile = t0; tile < t1; ++tile) {
+    if (tile >= tab.prefix[pos + 1]) {
+      flush(pos);
+      while (tile >= tab.prefix[pos + 1]) ++pos;
+      load_coef(pos);
+    }
+    const long long left = tab.lay[pos].pad - (tile - tab.prefix[pos]) * TF;
+    const bool live = (long long)(VEC * tid) < left;                    // pad % 32 == 0, VEC | 32: all or nothing
+    const float *row0 = ring + (size_t)s * K * TF + VEC * tid;
+    mbar_wait(full + s, ph);
+    if (KEEP) {
+      double xd[KT][VEC], m[VEC];
+#pragma unroll
+      for (int v = 0; v < VEC; ++v) m[v] = 0.0;
+#pragma unroll
+      for (int i = 0; i < KT; ++i) {
+        float xv[VEC];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) xv[v] = 0.f;
+        const double ci = weighted ? (i < K ? coef[i] : 0.0) : inv_k;
+        if (i < K && live) {
+          if (VEC == 2) { const float2 t = *reinterpret_cast<const float2 *>(row0 + (size_t)i * TF); xv[0] = t.x; xv[1] = t.y; }
+          else xv[0] = row0[(size_t)i * TF];
+        }
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+          xd[i][v] = (double)xv[v];
+          m[v] = fma(ci, xd[i][v], m[v]);
+        }
+      }
+      __syncwarp();
+      if ((tid & 31) == 0) mbar_arrive(empty + s);                      // the tile now lives in registers
+#pragma unroll
+      for (int i = 0; i < KT; ++i) {
+        if (i < K && live) {
+#pragma unroll
+          for (int v = 0; v < VEC; ++v) {
+            const double d = xd[i][v] - m[v];
+            acc[i] = fma(d, d, acc[i]);
+          }
+        }
+      }
+    } else {
+      double m[VEC];
+#pragma unroll
+      for (int v = 0; v < VEC; ++v) m[v] = 0.0;
+      if (live) {
+#pragma unroll
+        for (int i = 0; i < KT; ++i) {
+          if (i < K) {
+            const double ci = weighted ? coef[i] : inv_k;
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) m[v] = fma(ci, (double)row0[(size_t)i * TF + v], m[v]);
+          }
+        }
+#pragma unroll
+        for (int i = 0; i < KT; ++i) {
+          if (i < K) {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+              const double d = (double)row0[(size_t)i * TF + v] - m[v];
+              acc[i] = fma(d, d, acc[i]);
+            }
+          }
+        }
+      }
+      __syncwarp();
+      if ((tid & 31) == 0) mbar_arrive(empty + s);
+    }
+    if (++s == S) { s = 0; ph ^= 1u; }
+  }
+  flush(pos);
+}
+
+// ---- general form (K > 64): consensus of every column through shared memory, one or two stages
+constexpr int kGenThreads = 256;
 template <int MAXIT>
-__global__ void __launch_bounds__(kDiagThreads) layup_disagreement_kernel(const __grid_constant__ DiagParams p,
+__global__ void __launch_bounds__(kGenThreads) layup_disagreement_general(const __grid_constant__ DiagParams p,
                                                                           const __grid_constant__ PosTable tab) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr int THREADS = kDiagThreads;
+  constexpr int THREADS = kGenThreads;
   const int K = p.K, C = p.C, log2C = p.log2C, tid = threadIdx.x;
   const int n_items = K << log2C;
+  const bool two_stage = p.stages >= 2;
   float4 *stage0 = reinterpret_cast<float4 *>(smem_raw);                          // [1 or 2][K*C]
-  double *mean = reinterpret_cast<double *>(stage0 + (p.two_stage ? 2 : 1) * (size_t)n_items);   // [C*4]
-  double *psum = mean + 4 * C;                                                    // [THREADS*4] partial consensus sums
-  double *coef = psum + 4 * THREADS;                                              // [K]
+  double *mean = reinterpret_cast<double *>(stage0 + (two_stage ? 2 : 1) * (size_t)n_items);   // [C*4]
+  double *coef = mean + 4 * C;                                                    // [K]
   double *red = coef + K;                                                         // [K] per-layer CTA sums
   uint64_t *bars = reinterpret_cast<uint64_t *>(red + K);                         // [2]
 
@@ -99,8 +279,8 @@ __global__ void __launch_bounds__(kDiagThreads) layup_disagreement_kernel(const 
   if (tile < n_tiles) issue_load(tile, 0);
   int cur = -1;
   for (int it = 0; tile < n_tiles; tile += gridDim.x, ++it) {
-    const int s = p.two_stage ? (it & 1) : 0;
-    if (p.two_stage && tile + gridDim.x < n_tiles) issue_load(tile + gridDim.x, s ^ 1);   // prefetch into the free stage
+    const int s = two_stage ? (it & 1) : 0;
+    if (two_stage && tile + gridDim.x < n_tiles) issue_load(tile + gridDim.x, s ^ 1);   // prefetch into the free stage
     const int pos = locate(tile);
     if (pos != cur) {
       // leaving a layer: flush this CTA's partial sums, load the next layer's coefficients
@@ -115,52 +295,9 @@ __global__ void __launch_bounds__(kDiagThreads) layup_disagreement_kernel(const 
     const long long cols_left = (pad >> 2) - col0;
     const int ncols = cols_left < C ? (int)cols_left : C;
     const float4 *xs = stage0 + (size_t)s * n_items;
-    mbar_wait(bars + s, (uint32_t)(p.two_stage ? (it >> 1) : it) & 1u);
+    mbar_wait(bars + s, (uint32_t)(two_stage ? (it >> 1) : it) & 1u);
 
-    if (MAXIT <= 8 && C <= THREADS) {
-      // Fast form: fp32 -> fp64 conversion is the scarce resource here (16 per clock and SM), so every
-      // element is converted ONCE and kept in registers for both the consensus and the distance.
-      // C divides THREADS: all items of a thread share the column c = tid & (C-1); the replicas of that
-      // column are spread over the THREADS/C thread groups g = tid >> log2C, which exchange their
-      // partial weighted sums through shared memory.
-      double xd[MAXIT][4];
-      double p0 = 0.0, p1 = 0.0, p2 = 0.0, p3 = 0.0;
-      const int c = tid & (C - 1);
-#pragma unroll
-      for (int u = 0; u < MAXIT; ++u) {
-        const int idx = u * THREADS + tid;
-        float4 v = float4{0.f, 0.f, 0.f, 0.f};
-        double ci = 0.0;
-        if (idx < n_items && c < ncols) {
-          v = xs[idx];
-          ci = coef[idx >> log2C];
-        }
-        xd[u][0] = (double)v.x; xd[u][1] = (double)v.y; xd[u][2] = (double)v.z; xd[u][3] = (double)v.w;
-        p0 += ci * xd[u][0]; p1 += ci * xd[u][1]; p2 += ci * xd[u][2]; p3 += ci * xd[u][3];
-      }
-      double *mine = psum + 4 * tid;                       // psum[g][c][4] with g*C + c == tid
-      mine[0] = p0; mine[1] = p1; mine[2] = p2; mine[3] = p3;
-      __syncthreads();
-      double m0 = 0.0, m1 = 0.0, m2 = 0.0, m3 = 0.0;
-      for (int g = 0; g < (THREADS >> log2C); ++g) {
-        const double *q = psum + 4 * ((g << log2C) + c);
-        m0 += q[0]; m1 += q[1]; m2 += q[2]; m3 += q[3];
-      }
-#pragma unroll
-      for (int u = 0; u < MAXIT; ++u) {
-        const int idx = u * THREADS + tid;
-        if (idx < n_items && c < ncols) {
-          const double d0 = xd[u][0] - m0, d1 = xd[u][1] - m1, d2 = xd[u][2] - m2, d3 = xd[u][3] - m3;
-          acc[u] += d0 * d0 + d1 * d1 + d2 * d2 + d3 * d3;
-        }
-      }
-      fence_proxy_async();
-      __syncthreads();   // this stage and psum[] are reused
-      if (!p.two_stage && tile + gridDim.x < n_tiles) issue_load(tile + gridDim.x, 0);
-      continue;
-    }
-
-    // general form (very large K): consensus of every column, then the distances, both out of shared memory
+    // consensus of every column, then the distances, both out of shared memory
     // (pads are zero in every replica and contribute 0)
     for (int c = tid; c < ncols; c += THREADS) {
       double m0 = 0.0, m1 = 0.0, m2 = 0.0, m3 = 0.0;
@@ -187,31 +324,80 @@ __global__ void __launch_bounds__(kDiagThreads) layup_disagreement_kernel(const 
     }
     fence_proxy_async();
     __syncthreads();   // this stage and mean[] are reused
-    if (!p.two_stage && tile + gridDim.x < n_tiles) issue_load(tile + gridDim.x, 0);
+    if (!two_stage && tile + gridDim.x < n_tiles) issue_load(tile + gridDim.x, 0);
   }
   if (cur >= 0) flush(cur);
 }
 
+using DiagFn = void (*)(const DiagParams, const PosTable);
+struct RingShape {
+  int kt, vec, minb;
+  DiagFn fn;
+};
+// one CTA per SM: the registers go to the per-replica accumulators (and the fp64 copy of the tile),
+// the shared memory to a deep ring
+const RingShape kRing[] = {
+    {8, 2, 1, layup_disagreement_kernel<8, 2, true, 1>},
+    {16, 2, 1, layup_disagreement_kernel<16, 2, true, 1>},
+    {32, 2, 1, layup_disagreement_kernel<32, 2, false, 1>},
+    {64, 1, 1, layup_disagreement_kernel<64, 1, false, 1>},
+};
+const RingShape *ring_shape(int K) {
+  for (const RingShape &r : kRing)
+    if (K <= r.kt) return &r;
+  return nullptr;
+}
+
+size_t ring_smem(int K, int tf, int stages, int kt) {
+  return (size_t)stages * K * tf * sizeof(float) + 16 * (size_t)stages + sizeof(double) * (kConsumers / 32) * (size_t)kt;
+}
+size_t general_smem(int K, int C, bool two_stage) {
+  return (two_stage ? 2 : 1) * (size_t)K * C * sizeof(float4) + sizeof(double) * (4 * (size_t)C + 2 * (size_t)K) + 16;
+}
+int general_iters(int K, int C) { return (K * C + kGenThreads - 1) / kGenThreads; }
+
 }  // namespace
 
-size_t diag_smem_bytes(int K, int C, bool two_stage) {
-  return (two_stage ? 2 : 1) * (size_t)K * C * sizeof(float4) + sizeof(double) * (4 * (size_t)C + 4 * kDiagThreads + 2 * (size_t)K) + 16;
-}
-
-static int diag_iters(int K, int C) { return (K * C + kDiagThreads - 1) / kDiagThreads; }
-
-cudaError_t diag_setup(int K, int C, int smem_bytes, int *ctas_per_sm) {
+// Picks the kernel shape for K: *C = float4 columns per tile, *stages = ring depth (general kernel: 1 or 2).
+cudaError_t diag_plan(int K, size_t smem_optin, int *C, int *stages, int *smem_bytes, int *ctas_per_sm) {
   cudaError_t e;
-  auto f = diag_iters(K, C) <= 8 ? layup_disagreement_kernel<8> : layup_disagreement_kernel<32>;
-  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, f, kDiagThreads, smem_bytes);
+  if (const RingShape *r = ring_shape(K)) {
+    const int tf = kConsumers * r->vec;
+    // as deep as fits: minb CTAs share ~224 KB of shared memory per SM
+    const size_t budget = (size_t)(224 * 1024) / r->minb - 1024 - sizeof(double) * (kConsumers / 32) * r->kt;
+    int S = (int)((budget < smem_optin ? budget : smem_optin) / ((size_t)K * tf * sizeof(float) + 16));
+    if (S > 8) S = 8;
+    if (S >= 2) {
+      *C = tf / 4;
+      *stages = S;
+      *smem_bytes = (int)ring_smem(K, tf, S, r->kt);
+      if ((e = cudaFuncSetAttribute(r->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, *smem_bytes)) != cudaSuccess) return e;
+      if ((e = cudaFuncSetAttribute(r->fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
+      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, r->fn, kRingThreads, *smem_bytes);
+    }
+  }
+  int c = 8;
+  while ((long long)K * c * 2 <= 2048 && c < 256) c *= 2;
+  const bool two = general_smem(K, c, true) <= smem_optin;
+  *C = c;
+  *stages = two ? 2 : 1;
+  *smem_bytes = (int)general_smem(K, c, two);
+  if (general_iters(K, c) > 32) return cudaErrorInvalidValue;
+  auto f = general_iters(K, c) <= 8 ? layup_disagreement_general<8> : layup_disagreement_general<32>;
+  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, *smem_bytes)) != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, f, kGenThreads, *smem_bytes);
 }
 
-cudaError_t launch_disagreement(const float *x, const double *w, double *dist, int K, int C, int log2C, bool two_stage,
+cudaError_t launch_disagreement(const float *x, const double *w, double *dist, int K, int C, int log2C, int stages,
                                 const PosTable &tab, int grid, int smem_bytes, cudaStream_t s) {
-  DiagParams p{x, w, dist, K, C, log2C, two_stage ? 1 : 0};
-  if (diag_iters(K, C) <= 8) layup_disagreement_kernel<8><<<grid, kDiagThreads, smem_bytes, s>>>(p, tab);
-  else if (diag_iters(K, C) <= 32) layup_disagreement_kernel<32><<<grid, kDiagThreads, smem_bytes, s>>>(p, tab);
+  DiagParams p{x, w, dist, K, C, log2C, stages};
+  const RingShape *r = ring_shape(K);
+  if (r && C * 4 == kConsumers * r->vec && stages >= 2 && (size_t)smem_bytes == ring_smem(K, C * 4, stages, r->kt)) {
+    r->fn<<<grid, kRingThreads, smem_bytes, s>>>(p, tab);
+    return cudaGetLastError();
+  }
+  if (general_iters(K, C) <= 8) layup_disagreement_general<8><<<grid, kGenThreads, smem_bytes, s>>>(p, tab);
+  else if (general_iters(K, C) <= 32) layup_disagreement_general<32><<<grid, kGenThreads, smem_bytes, s>>>(p, tab);
   else return cudaErrorInvalidValue;
   return cudaGetLastError();
 }

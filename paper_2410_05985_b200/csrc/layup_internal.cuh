@@ -39,7 +39,7 @@ struct SchedParams {
   SchedTables t;
   double *w;                // [L*K] push-sum weights, updated in place
   uint64_t seed;
-  uint32_t step;
+  uint32_t *step_dev;       // [L] the round each layer runs next: read, then advanced, by the schedule stage
   uint32_t skip_thr;        // skip iff draw < skip_thr; 0 = straggler mode off
   int32_t K, L;
   int32_t layer_begin;      // blockIdx.x + layer_begin = layer
@@ -68,7 +68,17 @@ struct UpdateParams {
   int32_t all_active;               // skip_prob == 0: every replica is active in every round
   SchedParams sched;                // fused single-launch path: the schedule stage's inputs
   const void *tmaps;                // [n_sections][L] CUtensorMap (128 B each) of the layer sections, or nullptr
+  unsigned long long *trace;        // [L] first CTA start per layer (%globaltimer, atomicMin), or nullptr (layup_trace)
 };
+
+// layup_trace: the first CTA of a (step, layer) event to start leaves the GPU nanosecond timer
+__device__ __forceinline__ void trace_start(unsigned long long *trace, int layer) {
+  if (trace != nullptr && threadIdx.x == 0) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    atomicMin(trace + layer, t);
+  }
+}
 
 // Work-list table of one launch, passed by value in the kernel parameters (constant bank):
 // the launch covers positions [0, n) of this table; position q holds layer `layer[q]`
@@ -87,9 +97,8 @@ cudaError_t launch_peers_only(uint64_t seed, uint32_t step, uint32_t skip_thr, i
                               int delay_replica, int delay_rounds, int32_t *peer_dev, unsigned char *active_dev,
                               cudaStream_t s);
 // diagnose.cu
-size_t diag_smem_bytes(int K, int C, bool two_stage);
-cudaError_t diag_setup(int K, int C, int smem_bytes, int *ctas_per_sm);
-cudaError_t launch_disagreement(const float *x, const double *w, double *dist, int K, int C, int log2C, bool two_stage,
+cudaError_t diag_plan(int K, size_t smem_optin, int *C, int *stages, int *smem_bytes, int *ctas_per_sm);
+cudaError_t launch_disagreement(const float *x, const double *w, double *dist, int K, int C, int log2C, int stages,
                                 const PosTable &tab, int grid, int smem_bytes, cudaStream_t s);
 // update.cu
 int update_num_variants();
@@ -105,10 +114,12 @@ cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_byte
 cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, bool pdl, int grid,
                               int smem_bytes, cudaStream_t s);
 
-// update_persist.cu -- persistent two-stage form (LAYUP_PERSISTENT=1)
-size_t persist_smem_bytes(int K, int C, int opt);
-cudaError_t persist_kernel_setup(int opt, int smem_bytes, int *ctas_per_sm);
-cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, int grid, int smem_bytes, bool pdl,
-                                  cudaStream_t s);
+// update_persist.cu -- persistent warp-specialised ring form (layup_tuning.launch_shape = 2)
+int persist_max_k();
+int persist_stages(int K, int C, int opt, size_t smem_optin, int ctas, int want);
+size_t persist_smem_bytes(int K, int C, int opt, int stages);
+cudaError_t persist_kernel_setup(int opt, bool symmetric, int smem_bytes, int *ctas_per_sm);
+cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, int grid, int smem_bytes, int stages,
+                                  bool pdl, cudaStream_t s);
 
 }  // namespace layup

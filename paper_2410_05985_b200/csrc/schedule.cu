@@ -31,14 +31,17 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
   const int layer = p.layer_begin + blockIdx.x;
   const int i = threadIdx.x;
   const size_t row = (size_t)layer * K;
+  // the round number is device state (layup.h "CUDA-graph capture"): every thread reads it here,
+  // thread 0 advances it after the barrier below
+  const uint32_t step = p.step_dev[layer];
 
   bool act = false;
   if (i < K) {
-    act = draw_active(p.seed, p.step, i, p.skip_thr, p.delay_replica, p.delay_rounds);
+    act = draw_active(p.seed, step, i, p.skip_thr, p.delay_replica, p.delay_rounds);
     int peer = -1;
     double wh = p.w[row + i];
     if (act && K >= 2) {
-      peer = draw_peer(p.seed, p.step, p.peer_mode == 0 ? (uint32_t)layer : kNoLayer, i, K);
+      peer = draw_peer(p.seed, step, p.peer_mode == 0 ? (uint32_t)layer : kNoLayer, i, K);
       if (p.mix_mode != kMixSymmetric) wh = wh * 0.5;            // w_i <- w_i / 2 (exact)
     }
     if (p.adamw && act) {                                        // this worker takes its t-th step
@@ -54,6 +57,7 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
     p.t.peer[row + i] = peer;
   }
   __syncthreads();
+  if (i == 0) p.step_dev[layer] = step + 1u;
 
   // CSR by receiver without a serial prefix sum: the senders of receivers below i are exactly the
   // pushes whose peer index is below i; one pass over the K peers gives count, offset and last writer

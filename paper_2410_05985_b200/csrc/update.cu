@@ -147,6 +147,7 @@ __global__ void __launch_bounds__(THREADS, MINB) layup_update_grouped(const Upda
     if (tile >= p.tile_prefix[mid]) lo = mid; else hi = mid;
   }
   const int layer = p.L - 1 - lo;
+  trace_start(p.trace, layer);
   load_schedule<OPT, SYM, THREADS>(p, s, layer);
   const LayerDesc lay = p.layers[layer];
   const long long t_in = tile - p.tile_prefix[lo];
@@ -165,6 +166,7 @@ __global__ void __launch_bounds__(THREADS, MINB) layup_update_persistent(const U
     while (tile >= pos_end_tile) { ++pos; pos_end_tile = p.tile_prefix[pos + 1]; }
     const int layer = p.L - 1 - pos;
     if (pos != loaded_pos) {
+      trace_start(p.trace, layer);
       load_schedule<OPT, SYM, THREADS>(p, s, layer);
       loaded_pos = pos;
       __syncthreads();

@@ -1,14 +1,24 @@
 // Persistent form of the TMA-staged update kernel: a fixed grid of resident CTAs drains the
 // reverse-layer-ordered work list (BASELINE.json north_star item 3, "a persistent grouped launch
-// that drains many small layers from a work list") with a two-stage shared-memory pipeline: while
-// a CTA computes and stores tile n out of one stage, the TMA engine fills the other stage with
-// tile n + gridDim.x.  Same work item, same arithmetic (rule.cuh) and the same bits as
-// update_tma.cu; the layer's schedule tables are reloaded only when the CTA crosses into another
-// layer.
+// that drains many small layers from a work list"; the per-layer event of PAPER.md:108-112 is most
+// frequent exactly there).  Same work item, same arithmetic (rule.cuh) and the same bits as
+// update_tma.cu.  Selected with layup_tuning.launch_shape = 2.
 //
-// Scope: every replica active, sender-list mixers (push-sum, lossy), schedule tables from the
-// schedule kernel.  It is selected with LAYUP_PERSISTENT=1: on B200 the one-CTA-per-work-item
-// launch measures faster, so this form is the measured alternative, not the default.
+// Warp-specialised: every CTA is ONE producer warp plus kPsConsumers consumer threads around an
+// S-stage shared-memory ring (S >= 2, as deep as fits; layup_tuning.stages).
+//   producer  walks the CTA's share of the list (tile = blockIdx.x + n*gridDim.x, so the list is
+//             drained in order, output layer first); for each tile it waits for the stage's
+//             "empty" mbarrier, copies the layer's schedule tables (held in its registers, reloaded
+//             only when the list crosses into another layer) into the stage, and issues the tile's
+//             TMA loads on the stage's "full" mbarrier: ONE 2-D tiled load per array when every
+//             replica is active, else 1-D bulk copies of exactly the rows the flags ask for
+//             (an idle replica costs nothing, an idle receiver only its x row) -- the flags are in
+//             the producer's registers, so a straggler round's loads need no table round trip;
+//   consumers wait for "full", take the local steps out of shared memory (y overwrites x in place,
+//             m' / v' go to HBM), meet on a named barrier that only the consumer warps share, fold
+//             every receiver's senders and write x once, then release the stage ("empty").  No
+//             CTA-wide barrier exists, so the producer is never gated by the consumers' phases:
+//             up to S-1 tiles are in flight while one is computed.
 #include "layup_internal.cuh"
 #include "rule.cuh"
 #include "tma_ptx.cuh"
@@ -17,161 +27,250 @@ namespace layup {
 
 namespace {
 
-constexpr int kPsThreads = 256;
+constexpr int kPsConsumers = 256;
+constexpr int kPsThreads = kPsConsumers + 32;
+constexpr int kPsMaxEntries = 4;                      // table entries per producer lane: K <= 128
 
-template <int OPT>
-__global__ void __launch_bounds__(kPsThreads, 2)
-    layup_update_persist(const __grid_constant__ UpdateParams p, const __grid_constant__ PosTable tab) {
+__device__ __forceinline__ void ps_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void consumer_barrier() {
+  asm volatile("bar.sync 1, %0;" ::"n"(kPsConsumers) : "memory");
+}
+
+// per-stage copy of a layer's schedule (what the consumers read)
+struct StageTables {
+  int *begin, *cnt, *senders;
+  float *alpha, *c1, *c2;
+  unsigned char *flags;
+};
+__host__ __device__ inline size_t tables_bytes(int K) { return ((size_t)K * 25 + 15) / 16 * 16; }
+__device__ __forceinline__ StageTables carve_tables(unsigned char *base, int K) {
+  StageTables t;
+  t.begin = reinterpret_cast<int *>(base);
+  t.cnt = t.begin + K;
+  t.senders = t.cnt + K;
+  t.alpha = reinterpret_cast<float *>(t.senders + K);
+  t.c1 = t.alpha + K;
+  t.c2 = t.c1 + K;
+  t.flags = reinterpret_cast<unsigned char *>(t.c2 + K);
+  return t;
+}
+
+template <int OPT, bool SYM>
+__global__ void __launch_bounds__(kPsThreads, 1)
+    layup_update_persist(const __grid_constant__ UpdateParams p, const __grid_constant__ PosTable tab, const int S) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int NARR = OptTraits<OPT>::kArrays;
   constexpr bool HAS_M = NARR >= 3, HAS_V = NARR >= 4;
-  constexpr int THREADS = kPsThreads;
   const int K = p.K, C = p.C, log2C = p.log2C, tid = threadIdx.x;
   const int n_items = K << log2C;
   const size_t stage_f4 = (size_t)NARR * n_items;                            // float4 per stage
-  float4 *stage0 = reinterpret_cast<float4 *>(smem_raw);
-  uint64_t *bars = reinterpret_cast<uint64_t *>(stage0 + 2 * stage_f4);      // [2] one per stage
-  int *s_begin = reinterpret_cast<int *>(bars + 2);                          // [K]
-  int *s_cnt = s_begin + K;
-  int *s_senders = s_cnt + K;
-  float *s_alpha = reinterpret_cast<float *>(s_senders + K);
-  float *s_c1 = s_alpha + K;                                                 // [K] (AdamW only)
-  float *s_c2 = s_c1 + (HAS_V ? K : 0);
-
-  const long long n_tiles = tab.prefix[tab.n];
-  const bool boxed = p.tmaps != nullptr;
-  constexpr int NW = THREADS / 32;
-  const int slot0 = (tid & 31) * NW + (tid >> 5);
-
-  auto locate = [&](long long tile) {
-    int lo = 0, hi = tab.n;
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (tile >= tab.prefix[mid]) lo = mid; else hi = mid;
-    }
-    return lo;
-  };
-  // request tile `tile` into stage `s` (all threads call it; the copies are spread over the warps)
-  auto issue_load = [&](long long tile, int s) {
-    const int lo = locate(tile);
-    const long long pad = tab.lay[lo].pad;
-    const long long col0 = (tile - tab.prefix[lo]) << log2C;
-    const long long cols_left = (pad >> 2) - col0;
-    const uint32_t chunk = (uint32_t)(cols_left < C ? cols_left : C) * 16u;
-    float4 *st = stage0 + (size_t)s * stage_f4;
-    uint64_t *bar = bars + s;
-    if (boxed) {
-      if (tid == 0) {
-        mbar_expect_tx(bar, (uint32_t)n_items * 16u * NARR);
-        const unsigned char *tm = reinterpret_cast<const unsigned char *>(p.tmaps);
-#pragma unroll
-        for (int a = 0; a < NARR; ++a)
-          tma_load_2d(st + a * n_items, tm + ((size_t)a * p.L + tab.layer[lo]) * 128, (int)(col0 << 2), 0, bar);
-      }
-    } else {
-      if (tid == 0) mbar_expect_tx(bar, (uint32_t)K * NARR * chunk);
-      const long long tile_off = tab.lay[lo].base + (col0 << 2);
-      for (int c = slot0; c < K * NARR; c += THREADS) {
-        const int i = c / NARR, a = c - i * NARR;
-        const float *src = (a == 0 ? p.x : a == 1 ? p.g : a == 2 ? p.m : p.v) + tile_off + (long long)i * pad;
-        bulk_g2s(st + a * n_items + (i << log2C), src, chunk, bar);
-      }
-    }
-  };
+  float4 *ring = reinterpret_cast<float4 *>(smem_raw);                       // [S][NARR][K*C]
+  uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)S * stage_f4);    // [S]
+  uint64_t *empty = full + S;                                                // [S]
+  unsigned char *tables0 = reinterpret_cast<unsigned char *>(empty + S);     // [S] StageTables
+  const size_t tb = tables_bytes(K);
 
   if (tid == 0) {
-    mbar_init(bars, 1);
-    mbar_init(bars + 1, 1);
+    for (int s = 0; s < S; ++s) {
+      mbar_init(full + s, 1);
+      mbar_init(empty + s, kPsConsumers / 32);
+    }
   }
-  __syncthreads();   // mbarriers visible
+  __syncthreads();   // the only CTA-wide barrier: mbarriers visible
 
-  long long tile = blockIdx.x;
-  if (tile < n_tiles) issue_load(tile, 0);
-  int cur_layer = -1;
-  for (int it = 0; tile < n_tiles; tile += gridDim.x, ++it) {
-    const int s = it & 1;
-    // the other stage was released by the barrier that closed the previous iteration: prefetch
-    if (tile + gridDim.x < n_tiles) issue_load(tile + gridDim.x, s ^ 1);
+  const long long n_tiles = tab.prefix[tab.n];
 
-    const int lo = locate(tile);
-    const int layer = tab.layer[lo];
-    const long long pad = tab.lay[lo].pad;
-    const long long col0 = (tile - tab.prefix[lo]) << log2C;
+  if (tid >= kPsConsumers) {
+    // ------------------------------------------------------------------ producer warp
+    const int lane = tid - kPsConsumers;
+    const bool boxed = p.all_active && p.tmaps != nullptr;
+    int r_begin[kPsMaxEntries], r_cnt[kPsMaxEntries], r_send[kPsMaxEntries], r_flag[kPsMaxEntries];
+    float r_alpha[kPsMaxEntries], r_c1[kPsMaxEntries], r_c2[kPsMaxEntries];
+    int pos = 0, cur_pos = -1, s = 0;
+    uint32_t ph = 0;
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      while (tile >= tab.prefix[pos + 1]) ++pos;
+      if (pos != cur_pos) {
+        // the schedule kernel in front of this launch wrote the tables (programmatic dependent launch)
+        if (cur_pos < 0) asm volatile("griddepcontrol.wait;" ::: "memory");
+        const int layer = tab.layer[pos];
+        const size_t row = (size_t)layer * K;
+#pragma unroll
+        for (int e = 0; e < kPsMaxEntries; ++e) {
+          const int k = lane + 32 * e;
+          r_flag[e] = 0;
+          if (k < K) {
+            r_send[e] = SYM ? p.t.peer[row + k] : p.t.senders[row + k];
+            r_alpha[e] = p.t.alpha[row + k];
+            r_flag[e] = p.t.flags[row + k];
+            const int b = p.t.recv_off[(size_t)layer * (K + 1) + k];
+            r_begin[e] = b;
+            r_cnt[e] = p.t.recv_off[(size_t)layer * (K + 1) + k + 1] - b;
+            r_c1[e] = HAS_V ? p.t.c1[row + k] : 0.f;
+            r_c2[e] = HAS_V ? p.t.c2[row + k] : 0.f;
+          }
+        }
+        cur_pos = pos;
+      }
+      const long long pad = tab.lay[pos].pad;
+      const long long col0 = (tile - tab.prefix[pos]) << log2C;
+      const long long cols_left = (pad >> 2) - col0;
+      const uint32_t chunk = (uint32_t)(cols_left < C ? cols_left : C) * 16u;
+
+      mbar_wait(empty + s, ph ^ 1u);                      // the first trip round the ring is free
+      // hand the layer's tables to the consumers through the stage
+      const StageTables T = carve_tables(tables0 + (size_t)s * tb, K);
+      uint32_t bytes = 0;
+#pragma unroll
+      for (int e = 0; e < kPsMaxEntries; ++e) {
+        const int k = lane + 32 * e;
+        if (k < K) {
+          T.begin[k] = r_begin[e]; T.cnt[k] = r_cnt[e]; T.senders[k] = r_send[e]; T.alpha[k] = r_alpha[e];
+          if (HAS_V) { T.c1[k] = r_c1[e]; T.c2[k] = r_c2[e]; }
+          T.flags[k] = (unsigned char)r_flag[e];
+          bytes += r_flag[e] ? chunk * ((r_flag[e] & kFlagActive) ? (uint32_t)NARR : 1u) : 0u;
+        }
+      }
+      float4 *st = ring + (size_t)s * stage_f4;
+      if (boxed) {
+        __syncwarp();                                     // table stores of all lanes before lane 0's arrive (release)
+        if (lane == 0) {
+          mbar_expect_tx(full + s, (uint32_t)n_items * 16u * NARR);
+          const unsigned char *tm = reinterpret_cast<const unsigned char *>(p.tmaps);
+#pragma unroll
+          for (int a = 0; a < NARR; ++a)
+            tma_load_2d(st + a * n_items, tm + ((size_t)a * p.L + tab.layer[pos]) * 128, (int)(col0 << 2), 0, full + s);
+        }
+      } else {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xFFFFFFFFu, bytes, o);
+        __syncwarp();
+        if (lane == 0) mbar_expect_tx(full + s, bytes);
+        __syncwarp();
+        const long long tile_off = tab.lay[pos].base + (col0 << 2);
+#pragma unroll
+        for (int e = 0; e < kPsMaxEntries; ++e) {
+          const int i = lane + 32 * e;
+          if (i < K && r_flag[e]) {
+            const int na = (r_flag[e] & kFlagActive) ? NARR : 1;
+            for (int a = 0; a < na; ++a) {
+              const float *src = (a == 0 ? p.x : a == 1 ? p.g : a == 2 ? p.m : p.v) + tile_off + (long long)i * pad;
+              bulk_g2s(st + a * n_items + (i << log2C), src, chunk, full + s);
+            }
+          }
+        }
+      }
+      if (++s == S) { s = 0; ph ^= 1u; }
+    }
+    return;
+  }
+
+  // -------------------------------------------------------------------- consumer warps
+  constexpr int NT = kPsConsumers;
+  int pos = 0, cur_pos = -1, s = 0;
+  uint32_t ph = 0;
+  for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    while (tile >= tab.prefix[pos + 1]) ++pos;
+    if (pos != cur_pos) {
+      trace_start(p.trace, tab.layer[pos]);
+      cur_pos = pos;
+    }
+    const long long pad = tab.lay[pos].pad;
+    const long long col0 = (tile - tab.prefix[pos]) << log2C;
     const long long cols_left = (pad >> 2) - col0;
     const int ncols = cols_left < C ? (int)cols_left : C;
-    const long long tile_off = tab.lay[lo].base + (col0 << 2);
+    const long long tile_off = tab.lay[pos].base + (col0 << 2);
     float *const xb = p.x + tile_off;
     float *const mb = HAS_M ? p.m + tile_off : nullptr;
     float *const vb = HAS_V ? p.v + tile_off : nullptr;
-    if (layer != cur_layer) {
-      if (cur_layer < 0) asm volatile("griddepcontrol.wait;" ::: "memory");   // tables of the schedule kernel
-      const size_t row = (size_t)layer * K;
-      for (int k = tid; k < K; k += THREADS) {
-        s_senders[k] = p.t.senders[row + k];
-        s_alpha[k] = p.t.alpha[row + k];
-        const int b = p.t.recv_off[(size_t)layer * (K + 1) + k];
-        s_begin[k] = b;
-        s_cnt[k] = p.t.recv_off[(size_t)layer * (K + 1) + k + 1] - b;
-        if (HAS_V) {
-          s_c1[k] = p.t.c1[row + k];
-          s_c2[k] = p.t.c2[row + k];
-        }
-      }
-      cur_layer = layer;
-      __syncthreads();
-    }
-    float4 *xs = stage0 + (size_t)s * stage_f4, *gs = xs + n_items;
+    float4 *xs = ring + (size_t)s * stage_f4, *gs = xs + n_items;
     float4 *ms = HAS_M ? gs + n_items : gs, *vs = HAS_V ? ms + n_items : ms;
-    mbar_wait(bars + s, (uint32_t)(it >> 1) & 1u);
+    const StageTables T = carve_tables(tables0 + (size_t)s * tb, K);
+    mbar_wait(full + s, ph);                              // tile and tables have landed (acquire)
 
     // ---- phase 1: local step; y overwrites x in place, m' (v') -> HBM
-    for (int idx = tid; idx < n_items; idx += THREADS) {
+    for (int idx = tid; idx < n_items; idx += NT) {
       const int i = idx >> log2C, c = idx & (C - 1);
       if (c >= ncols) continue;
+      if (!(T.flags[i] & kFlagActive)) continue;          // idle replica: y = x already there (if it was loaded)
       float4 m = HAS_M ? ms[idx] : float4{0.f, 0.f, 0.f, 0.f};
       float4 v = HAS_V ? vs[idx] : float4{0.f, 0.f, 0.f, 0.f};
-      const float4 y = local_step4<OPT>(xs[idx], gs[idx], m, v, p.s, HAS_V ? s_c1[i] : 0.f, HAS_V ? s_c2[i] : 0.f);
+      const float4 y = local_step4<OPT>(xs[idx], gs[idx], m, v, p.s, HAS_V ? T.c1[i] : 0.f, HAS_V ? T.c2[i] : 0.f);
       const long long off = (long long)i * pad + (c << 2);
       if (HAS_M) st4(mb + off, m);
       if (HAS_V) st4(vb + off, v);
       xs[idx] = y;
     }
-    __syncthreads();
-    // ---- phase 2: each receiver folds its senders in ascending order; x written once
-    for (int idx = tid; idx < n_items; idx += THREADS) {
-      const int i = idx >> log2C, c = idx & (C - 1);
-      if (c >= ncols) continue;
-      float4 acc = xs[idx];
-      const int k0 = s_begin[i], k_end = k0 + s_cnt[i];
-      for (int k = k0; k < k_end; ++k) peer_update4(acc, xs[(s_senders[k] << log2C) + c], s_alpha[k]);
-      st4(xb + (long long)i * pad + (c << 2), acc);
+    consumer_barrier();
+    if (SYM) {
+      // ---- phase 2 (symmetric): every scalar column runs the K exchanges in worker order
+      float *ysf = reinterpret_cast<float *>(xs);
+      for (int e = tid; e < (ncols << 2); e += NT) symmetric_column(ysf, C << 2, e, K, T.senders);
+      consumer_barrier();
+      for (int idx = tid; idx < n_items; idx += NT) {
+        const int i = idx >> log2C, c = idx & (C - 1);
+        if (c >= ncols || !T.flags[i]) continue;          // idle and nobody's peer: 0 bytes
+        st4(xb + (long long)i * pad + (c << 2), xs[idx]);
+      }
+    } else {
+      // ---- phase 2: each receiver folds its senders in ascending order; x written once
+      for (int idx = tid; idx < n_items; idx += NT) {
+        const int i = idx >> log2C, c = idx & (C - 1);
+        if (c >= ncols) continue;
+        if (!T.flags[i]) continue;                        // idle, no push received: 0 bytes
+        float4 acc = xs[idx];
+        const int k0 = T.begin[i], k_end = k0 + T.cnt[i];
+        for (int k = k0; k < k_end; ++k) peer_update4(acc, xs[(T.senders[k] << log2C) + c], T.alpha[k]);
+        st4(xb + (long long)i * pad + (c << 2), acc);
+      }
     }
     fence_proxy_async();   // the stage was written through the generic proxy; the TMA engine refills it next
-    __syncthreads();       // this stage and the tables may be reused
+    __syncwarp();
+    if ((tid & 31) == 0) ps_arrive(empty + s);            // this warp is done with the stage
+    if (++s == S) { s = 0; ph ^= 1u; }
   }
 }
 
-using PsFn = void (*)(const UpdateParams, const PosTable);
-const PsFn kPs[3] = {layup_update_persist<OPT_SGD>, layup_update_persist<OPT_SGD_MOM>, layup_update_persist<OPT_ADAMW>};
+using PsFn = void (*)(const UpdateParams, const PosTable, const int);
+const PsFn kPs[3][2] = {{layup_update_persist<OPT_SGD, false>, layup_update_persist<OPT_SGD, true>},
+                        {layup_update_persist<OPT_SGD_MOM, false>, layup_update_persist<OPT_SGD_MOM, true>},
+                        {layup_update_persist<OPT_ADAMW, false>, layup_update_persist<OPT_ADAMW, true>}};
+
+size_t stage_bytes(int K, int C, int opt) {
+  const int narr = opt == OPT_ADAMW ? 4 : opt == OPT_SGD_MOM ? 3 : 2;
+  return (size_t)K * C * sizeof(float4) * narr + 16 + tables_bytes(K);
+}
 
 }  // namespace
 
-size_t persist_smem_bytes(int K, int C, int opt) {
-  const int narr = opt == OPT_ADAMW ? 4 : opt == OPT_SGD_MOM ? 3 : 2;
-  return 2 * (size_t)K * C * sizeof(float4) * narr + 16 + sizeof(int) * 3 * (size_t)K +
-         sizeof(float) * K * (opt == OPT_ADAMW ? 3 : 1);
+int persist_max_k() { return 32 * kPsMaxEntries; }
+
+// Ring depth: `want` stages if > 0, else as deep as `ctas` CTAs per SM allow (<= 8); 0 if fewer than 2 fit.
+int persist_stages(int K, int C, int opt, size_t smem_optin, int ctas, int want) {
+  if (ctas < 1) ctas = 1;
+  size_t budget = (size_t)(226 * 1024) / ctas - 1024;
+  if (budget > smem_optin) budget = smem_optin;
+  int S = (int)(budget / stage_bytes(K, C, opt));
+  if (S > 8) S = 8;
+  if (want > 0 && want < S) S = want;
+  return S >= 2 ? S : 0;
 }
 
-cudaError_t persist_kernel_setup(int opt, int smem_bytes, int *ctas_per_sm) {
+size_t persist_smem_bytes(int K, int C, int opt, int stages) { return stage_bytes(K, C, opt) * stages; }
+
+cudaError_t persist_kernel_setup(int opt, bool symmetric, int smem_bytes, int *ctas_per_sm) {
   if (opt < 0 || opt > 2) return cudaErrorInvalidValue;
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(kPs[opt], cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(kPs[opt], cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, kPs[opt], kPsThreads, smem_bytes);
+  PsFn f = kPs[opt][symmetric ? 1 : 0];
+  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, f, kPsThreads, smem_bytes);
 }
 
-cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, int grid, int smem_bytes, bool pdl,
-                                  cudaStream_t s) {
+cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, int grid, int smem_bytes, int stages,
+                                  bool pdl, cudaStream_t s) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
   cfg.blockDim = dim3((unsigned)kPsThreads);
@@ -182,7 +281,7 @@ cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, in
   attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, kPs[p.opt], p, tab);
+  return cudaLaunchKernelEx(&cfg, kPs[p.opt][p.symmetric ? 1 : 0], p, tab, stages);
 }
 
 }  // namespace layup

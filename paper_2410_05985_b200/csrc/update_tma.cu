@@ -72,6 +72,7 @@ __global__ void __launch_bounds__(THREADS, MINB)
   float *const vb = HAS_V ? p.v + tile_off : nullptr;
   const uint32_t chunk = (uint32_t)ncols * 16u;
 
+  trace_start(p.trace, layer);
   const bool boxed = p.all_active && p.tmaps != nullptr;   // whole-tile 2-D TMA loads, one per array
   if (tid == 0) {
     mbar_init(bar, 1);
@@ -113,14 +114,15 @@ __global__ void __launch_bounds__(THREADS, MINB)
     // the schedule stage itself (same arithmetic as layup_schedule_kernel, K <= THREADS)
     const SchedParams &q = p.sched;
     const size_t row = (size_t)layer * K;
+    const uint32_t step = q.step_dev[layer];                     // device state, advanced by the retiring CTA
     bool act = false;
     if (tid < K) {
       const int i = tid;
-      act = draw_active(q.seed, q.step, i, q.skip_thr, q.delay_replica, q.delay_rounds);
+      act = draw_active(q.seed, step, i, q.skip_thr, q.delay_replica, q.delay_rounds);
       int peer = -1;
       double wh = q.w[row + i];
       if (act && K >= 2) {
-        peer = draw_peer(q.seed, q.step, q.peer_mode == 0 ? (uint32_t)layer : kNoLayer, i, K);
+        peer = draw_peer(q.seed, step, q.peer_mode == 0 ? (uint32_t)layer : kNoLayer, i, K);
         if (!SYM) wh = wh * 0.5;                                 // w_i <- w_i / 2 (exact)
       }
       if (HAS_V) {
@@ -179,8 +181,13 @@ __global__ void __launch_bounds__(THREADS, MINB)
       s_wnew[j] = W;
       s_flags[j] = (unsigned char)((act ? kFlagActive : 0) | (cnt > 0 ? kFlagRecv : 0));
     }
-    __syncthreads();   // schedule visible; every read of w / bpow by this CTA has returned
-    if (tid == 0) ticket = atomicAdd(q.ticket + layer, 1);
+    __syncthreads();   // schedule visible; every read of step / w / bpow by this CTA has returned
+    if (tid == 0) {
+      // release: this CTA's reads of the old state are ordered before its ticket, so the CTA that
+      // draws the last ticket (acquire below) may overwrite the state
+      __threadfence();
+      ticket = atomicAdd(q.ticket + layer, 1);
+    }
   } else {
     // Programmatic dependent launch: this kernel may start while the schedule kernel in front of it
     // on the stream is still running (its tile loads above do not depend on it); the tables do.
@@ -261,7 +268,10 @@ __global__ void __launch_bounds__(THREADS, MINB)
     // state: it publishes the new push-sum weights / beta powers and re-arms the ticket
     __shared__ int s_last;
     const int tiles_in_layer = (int)(tab.prefix[lo + 1] - tab.prefix[lo]);
-    if (tid == 0) s_last = (ticket == tiles_in_layer - 1);
+    if (tid == 0) {
+      s_last = (ticket == tiles_in_layer - 1);
+      if (s_last) __threadfence();   // acquire: every other CTA's ticket (and its reads before it) is behind us
+    }
     __syncthreads();
     if (s_last) {
       const SchedParams &q = p.sched;
@@ -271,9 +281,29 @@ __global__ void __launch_bounds__(THREADS, MINB)
         if (HAS_V) {
           q.bpow[2 * (row + tid)] = s_bp[2 * tid];
           q.bpow[2 * (row + tid) + 1] = s_bp[2 * tid + 1];
+          if (s_flags[tid] & kFlagActive) {
+            q.t.c1[row + tid] = s_c1[tid];
+            q.t.c2[row + tid] = s_c2[tid];
+          }
         }
+        // the schedule this launch consumed, for layup_schedule_tables (same layout as schedule.cu)
+        q.t.peer[row + tid] = s_peer[tid];
+        q.t.flags[row + tid] = s_flags[tid];
+        // compact CSR by receiver (the lossy mixer keeps its one entry in slot j of shared memory)
+        const int b = s_begin[tid], n = SYM ? 0 : s_cnt[tid];
+        int off = 0;
+        for (int r = 0; r < tid && !SYM; ++r) off += s_cnt[r];
+        for (int k = 0; k < n; ++k) {
+          q.t.senders[row + off + k] = s_senders[b + k];
+          q.t.alpha[row + off + k] = s_alpha[b + k];
+        }
+        q.t.recv_off[(size_t)layer * (K + 1) + tid] = off;
+        if (tid == K - 1) q.t.recv_off[(size_t)layer * (K + 1) + K] = off + n;
       }
-      if (tid == 0) q.ticket[layer] = 0;
+      if (tid == 0) {
+        q.step_dev[layer] = q.step_dev[layer] + 1u;
+        q.ticket[layer] = 0;
+      }
     }
   }
 }

@@ -1,0 +1,311 @@
+"""Round-2 parity closures (pytest -m gpu, on the B200 box), all through the C-ABI:
+
+* EVERY element of EVERY layer of BASELINE.json configs[1] and configs[4] at full size, in the
+  launch configuration bench.py times (layup_round), against the oracle, bit for bit, for two
+  rounds; configs[2] (68 GB, more than the host oracle can hold) on whole layers wte, block 0,
+  block 23 and ln_f (SURVEY.md 8(d) "Oracle beside it");
+* the schedule tables the update kernel actually CONSUMED (layup_schedule_tables) against the
+  oracle's peer draw, active mask and fold coefficients, on the two-launch and single-launch paths;
+* the issue order of layup_round / layup_round_host (output layer first), from
+  the work list and from device timestamps;
+* work lists longer than one launch's table (L > 160);
+* CUDA-graph replay of recorded rounds (the round counter is device state)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from _util import compare, load_grads, make_pair, max_ulp
+from paper_2410_05985_b200 import (FUSED_AUTO, FUSED_NEVER, MIX_LOSSY, MIX_PUSHSUM, MIX_SYMMETRIC, OPT_ADAMW, OPT_SGD,
+                                   SHAPE_GROUPED, SHAPE_PERSISTENT, WHAT_G, WHAT_M, WHAT_X, LayUp)
+
+pytestmark = pytest.mark.gpu
+
+
+def _bits(a):
+    return np.ascontiguousarray(a).view(np.uint32)
+
+
+def _hbm_or_skip(w, sections):
+    free, _ = torch.cuda.mem_get_info()
+    need = w.K * sum((n + 31) // 32 * 32 for n in w.numel) * 4 * sections
+    if need + (8 << 30) > free:
+        pytest.skip("needs %.1f GB of HBM" % (need / 2**30))
+
+
+# ---------------------------------------------------------------- whole-layer parity, full size
+@pytest.mark.parametrize("name,rounds", [("gpt2s_k8", 2), ("manysmall_k64", 2)])
+def test_every_element_of_every_layer_full_size(name, rounds):
+    w = synth.workload(name)
+    _hbm_or_skip(w, 3)
+    lu = LayUp(w.K, w.numel, w.lr, w.momentum, w.seed, w.peer_mode, w.skip_prob)
+    ref = oracle.Oracle(w.numel, w.K, w.lr, w.momentum, w.seed, w.peer_mode, w.skip_prob)
+    for l in range(w.L):
+        synth.fill_init_(w, l, lu.view(WHAT_X, l))
+        ref.x[l][:] = lu.view(WHAT_X, l).cpu().numpy()
+    total = 0
+    for step in range(rounds):
+        for l in range(w.L):
+            synth.fill_grad_(w, step, l, lu.view(WHAT_G, l))
+        lu.layup_round(step)                                  # asynchronous; the oracle runs beside it
+        for l in reversed(range(w.L)):                        # the kernel does not write G
+            ref.layer_update(step, l, lu.view(WHAT_G, l).cpu().numpy())
+        lu.layup_sync()
+        for l in range(w.L):
+            got = lu.view(WHAT_X, l).cpu().numpy()
+            assert np.array_equal(_bits(got), _bits(ref.x[l])), (name, step, l, max_ulp(got, ref.x[l]))
+            total += got.size
+            if w.momentum != 0.0:
+                gm = lu.view(WHAT_M, l).cpu().numpy()
+                assert np.array_equal(_bits(gm), _bits(ref.m[l])), (name, step, l, "m")
+        assert np.array_equal(lu.layup_weights(), ref.w)
+    assert total == rounds * w.K * w.params_per_replica
+    print("%s: %d elements compared bit for bit over %d rounds" % (name, total, rounds))
+    lu.close()
+    del lu
+    torch.cuda.empty_cache()
+
+
+def test_whole_layers_of_configs2_full_size():
+    """configs[2] (K = 16 GPT-2 medium, 68 GB): the whole arena takes part in layup_round; wte,
+    every tensor of block 0 and of block 23, and ln_f are followed by the oracle layer by layer
+    (layers are independent given the schedule, which is keyed on the true layer index)."""
+    w = synth.workload("gpt2m_k16")
+    _hbm_or_skip(w, 3)
+    lu = LayUp(w.K, w.numel, w.lr, w.momentum, w.seed, w.peer_mode, w.skip_prob)
+    subset = [0] + list(range(2, 8)) + list(range(2 + 23 * 6, 2 + 24 * 6)) + [w.L - 1]
+    assert w.numel[0] == 50257 * 1024 and w.numel[w.L - 1] == 2048 and len(subset) == 14
+    state = {}
+    for l in range(w.L):
+        synth.fill_init_(w, l, lu.view(WHAT_X, l))
+        if l in subset:
+            x = lu.view(WHAT_X, l).cpu().numpy()
+            state[l] = (x, np.zeros_like(x), np.full(w.K, 1.0 / w.K))
+    total = 0
+    for step in range(2):
+        for l in range(w.L):
+            synth.fill_grad_(w, step, l, lu.view(WHAT_G, l))
+        lu.layup_round(step)
+        for l in reversed(subset):
+            x, m, wt = state[l]
+            oracle.layer_update(x, lu.view(WHAT_G, l).cpu().numpy(), m, wt, w.lr, w.momentum, w.seed, step, l,
+                                w.peer_mode, w.skip_prob)
+        lu.layup_sync()
+        wts = lu.layup_weights()
+        for l in subset:
+            x, m, wt = state[l]
+            assert np.array_equal(_bits(lu.view(WHAT_X, l).cpu().numpy()), _bits(x)), (step, l)
+            assert np.array_equal(_bits(lu.view(WHAT_M, l).cpu().numpy()), _bits(m)), (step, l, "m")
+            assert np.array_equal(wts[l], wt)
+            total += x.size
+    print("gpt2m_k16: %d elements of %d whole layers compared bit for bit" % (total, len(subset)))
+    lu.close()
+    del lu
+    torch.cuda.empty_cache()
+
+
+# ---------------------------------------------------------------- the tables the kernel consumed
+def _check_tables(lu, w, step, w_before, mix):
+    peer, active = oracle.schedule(w.seed, step, w.L, w.K, w.peer_mode, w.skip_prob)
+    for l in range(w.L):
+        t = lu.layup_schedule_tables(l)
+        assert t["step"] == step
+        assert np.array_equal(t["peer"], peer[l]), (step, l)
+        recv = np.array([((peer[l] == j) & (active == 1)).any() for j in range(w.K)])
+        assert np.array_equal(t["flags"], (active | (recv.astype(np.uint8) << 1)).astype(np.uint8)), (step, l)
+        off, snd, al, _ = oracle.mix_tables(w_before[l], peer[l], active, mix)
+        assert np.array_equal(t["recv_off"], off), (step, l)
+        n = int(off[-1])
+        if mix != MIX_SYMMETRIC:
+            assert np.array_equal(t["senders"][:n], snd) and np.array_equal(_bits(t["alpha"][:n]), _bits(al)), (step, l)
+
+
+@pytest.mark.parametrize("fused", [FUSED_AUTO, FUSED_NEVER])
+@pytest.mark.parametrize("mix", [MIX_PUSHSUM, MIX_LOSSY, MIX_SYMMETRIC])
+@pytest.mark.parametrize("K,skip", [(2, 0.0), (8, 0.25), (16, 0.0), (64, 0.25)])
+def test_consumed_schedule_tables_match_the_oracle(fused, mix, K, skip):
+    numel = [4097, 33, 800, 20000]
+    w = synth.Workload("tab", K, tuple(numel), 1e-2, 0.0, 5, 40 + K, skip_prob=skip)
+    lu = LayUp(K, numel, w.lr, 0.0, w.seed, 0, skip, mix_mode=mix, tuning=dict(fused=fused))
+    ref = oracle.Oracle(numel, K, w.lr, 0.0, w.seed, 0, skip, mix_mode=mix)
+    for l in range(w.L):
+        synth.fill_init_(w, l, lu.view(WHAT_X, l))
+        ref.x[l][:] = lu.view(WHAT_X, l).cpu().numpy()
+    n0 = lu.layup_launch_count()
+    for step in range(5):
+        grads = load_grads(w, lu, step)
+        w_before = ref.w.copy()
+        if step % 2 == 0:
+            lu.layup_round(step)
+        else:
+            for l in reversed(range(w.L)):
+                lu.layup_layer_update(step, l)
+        ref.round(step, grads)
+        _check_tables(lu, w, step, w_before, mix)
+        assert np.array_equal(lu.layup_weights(), ref.w)
+    assert lu.layup_launch_count() - n0 == (1 if fused == FUSED_AUTO else 2) * (3 + 2 * w.L)
+    lu.close()
+
+
+@pytest.mark.parametrize("name", ["gpt2m_k16", "manysmall_k64", "straggler_k8"])
+def test_consumed_tables_of_the_baseline_configs(name):
+    """K, L, seed, straggler probability of the BASELINE configs (tiny layers: the schedule does not
+    depend on numel); every round of the config, two-launch path as the large configs take it."""
+    w0 = synth.workload(name)
+    w = synth.shrink(w0, [64] * w0.L)
+    lu = LayUp(w.K, w.numel, w.lr, 0.0, w.seed, w.peer_mode, w.skip_prob, tuning=dict(fused=FUSED_NEVER))
+    ref = oracle.Oracle(w.numel, w.K, w.lr, 0.0, w.seed, w.peer_mode, w.skip_prob)
+    for step in range(min(w.rounds, 12)):
+        grads = load_grads(w, lu, step)
+        w_before = ref.w.copy()
+        lu.layup_round(step)
+        ref.round(step, grads)
+        _check_tables(lu, w, step, w_before, MIX_PUSHSUM)
+    lu.close()
+
+
+# ---------------------------------------------------------------- issue order
+@pytest.mark.parametrize("shape", [SHAPE_GROUPED, SHAPE_PERSISTENT])
+def test_round_issues_the_output_layer_first(shape):
+    """layup_round puts layer L-1 at the head of the work list and the device starts it first;
+    layers further down the list by more than a wave of work items start strictly later."""
+    numel = [3_000_000, 40, 2_000_000, 5_000_000, 1000, 4_000_000]
+    K = 8
+    lu = LayUp(K, numel, 1e-3, 0.9, 3, tuning=dict(launch_shape=shape, fused=FUSED_NEVER))
+    for l in range(len(numel)):
+        lu.view(WHAT_X, l).normal_(0, 0.02)
+        lu.view(WHAT_G, l).normal_(0, 1e-3)
+    lu.layup_round(0)
+    lu.layup_trace(True)
+    lu.layup_round(1)
+    first = lu.layup_trace_read().astype(np.int64)
+    lu.layup_trace(False)
+    L = len(numel)
+    assert lu.layup_last_order() == list(reversed(range(L)))
+    assert (first < np.iinfo(np.int64).max).all()
+    assert first[L - 1] == first.min()
+    tiles = [-(-((n + 31) // 32 * 8) // 128) for n in numel]          # C = 1024 / K float4 columns per tile
+    pos_start = np.cumsum([0] + [tiles[l] for l in reversed(range(L))])  # by position
+    for a in range(L):
+        for b in range(a + 1, L):
+            if pos_start[b] - pos_start[a] >= 4000:                     # > 6 waves of 592 resident CTAs apart
+                assert first[L - 1 - a] < first[L - 1 - b], (a, b, first)
+    lu.close()
+
+
+def test_round_host_issues_the_output_layer_first():
+    w = synth.shrink(synth.workload("gpt2s_k8"), synth.gpt2_layers(32, 128, 301, 16, 2))
+    lu = LayUp(w.K, w.numel, w.lr, w.momentum, w.seed)
+    total = w.K * sum(w.numel)
+    g_host = torch.randn(total).mul_(1e-3).pin_memory()
+    x_host = torch.empty(total).pin_memory()
+    lu.layup_round_host(0, g_host, x_host)
+    lu.layup_trace(True)
+    lu.layup_round_host(1, g_host, x_host)
+    first = lu.layup_trace_read().astype(np.int64)
+    assert lu.layup_last_order() == list(reversed(range(w.L)))
+    assert (np.diff(first) < 0).all(), first            # per-layer launches in stream order: strictly L-1 first
+    lu.layup_layer_update(2, 5)
+    assert lu.layup_last_order() == [5]
+    lu.close()
+
+
+# ---------------------------------------------------------------- long work lists
+@pytest.mark.parametrize("tuning", [dict(fused=FUSED_AUTO), dict(fused=FUSED_NEVER),
+                                    dict(fused=FUSED_NEVER, launch_shape=SHAPE_PERSISTENT)])
+def test_more_layers_than_one_launch_table(tuning):
+    """L = 401 > 160 positions per launch: the work list is split into consecutive launches."""
+    rng = np.random.default_rng(0)
+    numel = [int(v) for v in rng.integers(1, 3000, 401)]
+    w = synth.Workload("long", 8, tuple(numel), 1e-2, 0.9, 3, 7, skip_prob=0.2)
+    lu = LayUp(w.K, w.numel, w.lr, w.momentum, w.seed, 0, w.skip_prob, tuning=tuning)
+    ref = oracle.Oracle(w.numel, w.K, w.lr, w.momentum, w.seed, 0, w.skip_prob)
+    for l in range(w.L):
+        synth.fill_init_(w, l, lu.view(WHAT_X, l))
+        ref.x[l][:] = lu.view(WHAT_X, l).cpu().numpy()
+    n0 = lu.layup_launch_count()
+    for step in range(3):
+        grads = load_grads(w, lu, step)
+        lu.layup_round(step)
+        lu.layup_sync()
+        ref.round(step, grads)
+        _, u = compare(w, lu, ref, 1e-6, "L=401 step %d" % step)
+        assert u == 0
+        assert np.array_equal(lu.layup_weights(), ref.w)
+    per_round = (lu.layup_launch_count() - n0) // 3
+    assert per_round == (3 if tuning["fused"] == FUSED_AUTO else 4)      # ceil(401/160) update launches (+ schedule)
+    assert lu.layup_last_order() == list(reversed(range(401)))
+    lu.close()
+
+
+# ---------------------------------------------------------------- CUDA graphs
+@pytest.mark.parametrize("name", ["mlp3_k4", "straggler_k8"])
+@pytest.mark.parametrize("rounds_per_graph", [1, 3])
+def test_graph_replay_of_rounds_matches_the_oracle(name, rounds_per_graph):
+    """A recorded round (or three) replayed for later rounds: the round counter, the weights and
+    AdamW's powers are device state, so every replay draws the peers of ITS round."""
+    w = synth.workload(name)
+    lu, ref, _ = make_pair(w)
+    stream = torch.cuda.Stream()
+    # two ordinary rounds first, so that the capture starts from a non-trivial state
+    step = 0
+    for _ in range(2):
+        grads = load_grads(w, lu, step)
+        lu.layup_round(step); ref.round(step, grads); step += 1
+    lu.layup_sync()
+    lu.layup_graph_begin(stream)
+    for r in range(rounds_per_graph):
+        lu.layup_round(step + r, stream)                 # recorded, not run
+    g = lu.layup_graph_end()
+    compare(w, lu, ref)                                  # nothing ran during the capture
+    launches0 = lu.layup_launch_count()
+    for _ in range(4):
+        # one batch of gradients per replay (a replay of several rounds re-uses it, as the oracle does here)
+        grads = load_grads(w, lu, step)
+        stream.wait_stream(torch.cuda.current_stream())
+        lu.layup_graph_launch(g, stream)
+        for r in range(rounds_per_graph):
+            ref.round(step, grads); step += 1
+        lu.layup_sync()
+        _, u = compare(w, lu, ref, 1e-6, "%s graph replay to step %d" % (name, step))
+        assert u == 0
+        assert np.array_equal(lu.layup_weights(), ref.w)
+    assert lu.layup_launch_count() - launches0 == 4 * rounds_per_graph       # one fused kernel per round
+    # and ordinary calls carry on from where the replays left the ctx
+    grads = load_grads(w, lu, step)
+    lu.layup_round(step); ref.round(step, grads)
+    _, u = compare(w, lu, ref)
+    assert u == 0
+    lu.layup_graph_destroy(g)
+    lu.close()
+
+
+def test_graph_of_per_layer_events_adamw():
+    """One backward's worth of per-layer events (output layer first) as one graph, AdamW + two-launch path."""
+    adam = dict(weight_decay=0.01, beta1=0.9, beta2=0.95, eps=1e-8)
+    numel = [30000, 77, 5000, 12345]
+    w = synth.Workload("g", 8, tuple(numel), 1e-3, 0.0, 6, 21, grad_std=1e-3, skip_prob=0.25)
+    lu = LayUp(w.K, numel, w.lr, 0.0, w.seed, 1, w.skip_prob, optimizer=OPT_ADAMW, tuning=dict(fused=FUSED_NEVER), **adam)
+    ref = oracle.Oracle(numel, w.K, w.lr, 0.0, w.seed, 1, w.skip_prob, optimizer=OPT_ADAMW, **adam)
+    for l in range(w.L):
+        synth.fill_init_(w, l, lu.view(WHAT_X, l))
+        ref.x[l][:] = lu.view(WHAT_X, l).cpu().numpy()
+    stream = torch.cuda.Stream()
+    lu.layup_graph_begin(stream)
+    for l in reversed(range(w.L)):
+        lu.layup_layer_update(0, l, stream)
+    g = lu.layup_graph_end()
+    for step in range(5):
+        grads = load_grads(w, lu, step)
+        stream.wait_stream(torch.cuda.current_stream())
+        lu.layup_graph_launch(g, stream)
+        assert lu.layup_last_order() == list(reversed(range(w.L)))
+        ref.round(step, grads)
+        lu.layup_sync()
+        for l in range(w.L):
+            for what, want in ((WHAT_X, ref.x[l]), (WHAT_M, ref.m[l]), (3, ref.v[l])):
+                assert max_ulp(lu.view(what, l).cpu().numpy(), want) == 0, (step, l, what)
+        assert np.array_equal(lu.layup_weights(), ref.w)
+    lu.layup_graph_destroy(g)
+    lu.close()

@@ -35,10 +35,31 @@ def test_every_declared_symbol_is_exported(lib):
 def test_header_and_binding_structs_agree(lib):
     # the ctypes struct mirrors layup_config field by field
     text = open(os.path.join(ROOT, "include", "layup.h")).read()
-    body = re.search(r"typedef struct \{(.*?)\} layup_config;", text, flags=re.S).group(1)
+    body = re.search(r"typedef struct \{((?:(?!typedef struct).)*?)\} layup_config;", text, flags=re.S).group(1)
     body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
     names = re.findall(r"(\w+)\s*;", body)
     assert names == [f[0] for f in binding._Config._fields_]
+
+
+def test_tuning_block_is_the_only_switch(lib):
+    """layup_tuning (include/layup.h) mirrors the binding field by field, every field is documented
+    in the header, and the library reads no environment variable."""
+    text = open(os.path.join(ROOT, "include", "layup.h")).read()
+    body = re.search(r"typedef struct \{(.*?)\} layup_tuning;", text, flags=re.S).group(1)
+    fields = re.findall(r"int32_t\s+(\w+)\s*;\s*/\*", body)               # name followed by its comment
+    assert fields == [f[0] for f in binding._Tuning._fields_] and len(fields) == 10
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2410_05985_b200")):
+        for f in files:
+            if f.endswith((".cu", ".cuh", ".h", ".py")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "getenv" not in src and "os.environ" not in src.replace('os.environ.get("CUDA_HOME"', ""), f
+    # out-of-range tuning is an argument error, caught before any CUDA call
+    arr = (ctypes.c_int64 * 1)(100)
+    for bad in (dict(engine=3), dict(launch_shape=-1), dict(fused=5), dict(stages=-2)):
+        tune = binding._Tuning(**bad)
+        cfg = binding._Config(4, 1, arr, 0.01, 0.0, 0, 0, 0.0, 0, tuning=ctypes.pointer(tune))
+        n = ctypes.c_size_t()
+        assert lib.layup_arena_bytes(ctypes.byref(cfg), ctypes.byref(n)) == pkg.LAYUP_EINVAL
 
 
 def test_arena_bytes_layout():

@@ -93,12 +93,12 @@ def test_disagreement_full_size_and_bandwidth():
         want0 = ((x - (c[:, None] * x).sum(0, keepdim=True)) ** 2).sum(1).cpu().numpy()
         del x
         assert np.abs(got[0] - want0).max() <= 1e-9 * want0.max()
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
+    ms = []
     for _ in range(5):
         lu.layup_disagreement(False)
-    dt = (time.perf_counter() - t0) / 5
+        ms.append(lu.layup_disagreement_ms())           # device time of the reduction kernels (CUDA events)
+    dt = float(np.median(ms)) * 1e-3
     gbs = 4.0 * w.K * w.params_per_replica / dt / 1e9
-    print("layup_disagreement on configs[2]: %.2f ms per call, %.0f GB/s read (wall clock, incl. copy-out)" % (dt * 1e3, gbs))
-    assert gbs > 2000
+    print("layup_disagreement on configs[2]: %.3f ms per call on the device, %.0f GB/s read" % (dt * 1e3, gbs))
+    assert gbs > 4500
     lu.close()

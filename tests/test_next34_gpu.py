@@ -11,7 +11,7 @@ import torch
 import oracle
 import synth
 from _util import REL_TOL_100, REL_TOL_ROUND, max_ulp, rel_err
-from paper_2410_05985_b200 import (LAYUP_EINVAL, MIX_LOSSY, MIX_PUSHSUM, MIX_SYMMETRIC, OPT_ADAMW, OPT_SGD, WHAT_G,
+from paper_2410_05985_b200 import (ENGINE_LDG, FUSED_AUTO, FUSED_NEVER, SHAPE_GROUPED, SHAPE_PERSISTENT, LAYUP_EINVAL, MIX_LOSSY, MIX_PUSHSUM, MIX_SYMMETRIC, OPT_ADAMW, OPT_SGD, WHAT_G,
                                    WHAT_M, WHAT_V, WHAT_X, LayUp, LayUpError)
 
 pytestmark = pytest.mark.gpu
@@ -19,8 +19,8 @@ pytestmark = pytest.mark.gpu
 ADAM = dict(weight_decay=0.0031235, beta1=0.9, beta2=0.95, eps=1e-8)       # PAPER.md:469-480 + GPT-2 betas
 
 
-def _pair(K, numel, lr, mu, seed, skip, opt, mix, peer_mode=0, shadow=False, **kw):
-    lu = LayUp(K, numel, lr, mu, seed, peer_mode, skip, optimizer=opt, mix_mode=mix, **kw)
+def _pair(K, numel, lr, mu, seed, skip, opt, mix, peer_mode=0, shadow=False, tuning=None, **kw):
+    lu = LayUp(K, numel, lr, mu, seed, peer_mode, skip, optimizer=opt, mix_mode=mix, tuning=tuning, **kw)
     ref = oracle.Oracle(numel, K, lr, mu, seed, peer_mode, skip, optimizer=opt, mix_mode=mix, **kw)
     sh = oracle.Oracle(numel, K, lr, mu, seed, peer_mode, skip, optimizer=opt, mix_mode=mix, f64=True, **kw) if shadow else None
     w = synth.Workload("t", K, tuple(numel), lr, mu, 0, seed, grad_std=1e-3, heavy_frac=0.01, heavy_scale=100.0)
@@ -155,14 +155,12 @@ def test_layer_calls_equal_round_for_adamw():
 
 @pytest.mark.parametrize("opt,mix,K", [(OPT_ADAMW, MIX_PUSHSUM, 8), (OPT_ADAMW, MIX_SYMMETRIC, 8), (OPT_SGD, MIX_SYMMETRIC, 16),
                                        (OPT_ADAMW, MIX_PUSHSUM, 500)])
-def test_ldg_engine_covers_the_widened_rule(opt, mix, K, monkeypatch):
-    """The LDG kernels (large K, or LAYUP_ENGINE=0) implement the same optimisers and mixers.
+def test_ldg_engine_covers_the_widened_rule(opt, mix, K):
+    """The LDG kernels (large K, or layup_tuning.engine = 2) implement the same optimisers and mixers.
     K = 500 with AdamW does not fit the TMA staging and takes the LDG engine by itself."""
-    if K < 100:
-        monkeypatch.setenv("LAYUP_ENGINE", "0")
     kw = ADAM if opt == OPT_ADAMW else {}
     numel = NUMEL if K < 100 else [4097, 33, 800]
-    w, lu, ref, _ = _pair(K, numel, 1e-3, 0.0, 8, 0.2, opt, mix, **kw)
+    w, lu, ref, _ = _pair(K, numel, 1e-3, 0.0, 8, 0.2, opt, mix, tuning=dict(engine=ENGINE_LDG) if K < 100 else None, **kw)
     _run(w, lu, ref, None, 6)
     lu.close()
 
@@ -221,15 +219,14 @@ def test_argument_errors_of_the_new_fields():
                                              (OPT_ADAMW, MIX_PUSHSUM, 0.0, 0.25), (OPT_ADAMW, MIX_LOSSY, 0.0, 0.0),
                                              (OPT_ADAMW, MIX_SYMMETRIC, 0.0, 0.0)])
 @pytest.mark.parametrize("K", [1, 2, 5, 16, 64])
-def test_single_launch_path_equals_two_launch_path(opt, mix, mu, skip, K, monkeypatch):
+def test_single_launch_path_equals_two_launch_path(opt, mix, mu, skip, K):
     """Launch-latency-bound launches compute the schedule stage inside the update kernel (one
     launch per round / per layer event); larger ones run the schedule kernel first.  Same bits,
     same weights, and both equal the oracle."""
     kw = ADAM if opt == OPT_ADAMW else {}
     outs, launches = [], []
-    for fused in ("1", "0"):
-        monkeypatch.setenv("LAYUP_FUSED", fused)
-        w, lu, ref, _ = _pair(K, NUMEL, 1e-3, mu, 31, skip, opt, mix, **kw)
+    for fused in (FUSED_AUTO, FUSED_NEVER):
+        w, lu, ref, _ = _pair(K, NUMEL, 1e-3, mu, 31, skip, opt, mix, tuning=dict(fused=fused), **kw)
         n0 = lu.layup_launch_count()
         _run(w, lu, ref, None, 4)
         # per-layer events take the same path
@@ -316,19 +313,22 @@ def test_checkpoint_resume_is_bit_identical(opt):
 
 
 @pytest.mark.parametrize("K", [1, 3, 8, 16, 64, 100])
-@pytest.mark.parametrize("opt,mix,mu", [(OPT_SGD, MIX_PUSHSUM, 0.0), (OPT_SGD, MIX_LOSSY, 0.9), (OPT_ADAMW, MIX_PUSHSUM, 0.0)])
-def test_persistent_form_equals_grouped_form(K, opt, mix, mu, monkeypatch):
-    """LAYUP_PERSISTENT=1: resident CTAs drain the work list through a two-stage TMA pipeline.
-    Same bits as the one-CTA-per-work-item launch and as the oracle (LAYUP_FUSED=0 keeps these small
-    launches off the single-launch path so that the persistent kernel is the one that runs; a small
-    CTA cap forces every CTA through many tiles and several layers)."""
+@pytest.mark.parametrize("opt,mix,mu,skip", [(OPT_SGD, MIX_PUSHSUM, 0.0, 0.0), (OPT_SGD, MIX_LOSSY, 0.9, 0.0),
+                                             (OPT_ADAMW, MIX_PUSHSUM, 0.0, 0.0), (OPT_SGD, MIX_PUSHSUM, 0.9, 0.25),
+                                             (OPT_SGD, MIX_SYMMETRIC, 0.0, 0.25), (OPT_ADAMW, MIX_SYMMETRIC, 0.0, 0.0)])
+@pytest.mark.parametrize("stages", [0, 2])
+def test_persistent_form_equals_grouped_form(K, opt, mix, mu, skip, stages):
+    """layup_tuning.launch_shape = 2: resident CTAs drain the work list through a multi-stage TMA ring
+    (producer warp + consumer warps).  Same bits as the one-CTA-per-work-item launch and as the oracle,
+    for every mixer and for straggler rounds (fused = never keeps these small launches off the
+    single-launch path so that the persistent kernel is the one that runs; one CTA per SM forces
+    every CTA through many tiles and several layers; stages = 2 is the shallowest ring, the
+    default the deepest that fits)."""
     kw = ADAM if opt == OPT_ADAMW else {}
-    monkeypatch.setenv("LAYUP_FUSED", "0")
     outs = []
-    for persistent in ("1", "0"):
-        monkeypatch.setenv("LAYUP_PERSISTENT", persistent)
-        monkeypatch.setenv("LAYUP_CTAS_PER_SM", "1")
-        w, lu, ref, _ = _pair(K, NUMEL + [300000], 1e-3, mu, 61 + K, 0.0, opt, mix, **kw)
+    for shape in (SHAPE_PERSISTENT, SHAPE_GROUPED):
+        w, lu, ref, _ = _pair(K, NUMEL + [300000], 1e-3, mu, 61 + K, skip, opt, mix,
+                              tuning=dict(launch_shape=shape, fused=FUSED_NEVER, ctas_per_sm=1, stages=stages), **kw)
         _run(w, lu, ref, None, 3)
         outs.append([lu.view(WHAT_X, l).cpu().numpy().copy() for l in range(w.L)] + [lu.layup_weights()])
         lu.close()
