@@ -53,6 +53,15 @@ __global__ void __launch_bounds__(THREADS, MINB)
   float *s_c2 = s_c1 + (HAS_V ? K : 0);                                     // [K]  (AdamW only)
   unsigned char *s_flags = reinterpret_cast<unsigned char *>(s_c2 + (HAS_V ? K : 0));  // [K]
 
+  if (FUSED) {
+    // Launched as a programmatic dependent of whatever kernel precedes it on the stream (in a graph
+    // of L2-resident rounds: the previous round's launch of this same kernel): the CTAs are placed
+    // and set up while that kernel drains, and only here wait for it to complete -- everything this
+    // kernel reads (round counter, weights, x) may have been written by it.  The next launch may be
+    // staged from now on; it will wait for THIS grid at the same point.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  }
   // which layer does this work item belong to: binary search in the parameter table
   const long long tile = blockIdx.x;
   int lo = 0, hi = tab.n;
@@ -363,12 +372,9 @@ cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int va
   const TmaVariant &v = kTma[variant];
   TmaFn f = (fused ? v.fused : v.fn)[p.opt][p.symmetric ? 1 : 0];
   if (!f) return cudaErrorInvalidValue;
-  if (fused) {
-    f<<<grid, v.threads, smem_bytes, s>>>(p, tab);
-    return cudaGetLastError();
-  }
-  // after the schedule kernel on the same stream: programmatic stream serialization lets this
-  // kernel's prologue and tile loads overlap the schedule kernel (see griddepcontrol.wait above)
+  // two-launch path: behind the schedule kernel, programmatic stream serialization lets this kernel's
+  // prologue and tile loads overlap it (griddepcontrol.wait above guards the tables);
+  // single-launch path: the same attribute chains consecutive rounds (see the top of the kernel)
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
   cfg.blockDim = dim3((unsigned)v.threads);
