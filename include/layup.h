@@ -81,7 +81,8 @@ typedef struct {
                            schedule stage inside the update kernel (ONE launch); 2: never            */
   int32_t fused_waves;  /* default 4                                                                */
   int32_t tile_items;   /* float4 items (replicas x columns) per work item; default 1024            */
-  int32_t variant;      /* thread shape of the update kernel: 0 default, 1.. alternatives + 1       */
+  int32_t variant;      /* grouped shape: thread shape of the update kernel (index; 0 = default);
+                           persistent shape: consumer groups per CTA (0 = as many as the ring feeds) */
   int32_t ctas_per_sm;  /* cap on resident CTAs per SM of persistent grids; default: all that fit   */
   int32_t pdl;          /* 0 auto = 1; 1: the update kernel is a programmatic dependent launch behind
                            the schedule kernel; 2: plain stream order                               */

@@ -47,7 +47,7 @@ struct layup_ctx {
   int32_t *d_peer_scratch = nullptr, *d_ticket = nullptr;
   void *d_tmaps = nullptr;                // [n_sections][L] CUtensorMap: 2-D tiled view [K][pad] of every layer section
   bool ps_ok = false;                     // tuning.launch_shape == 2: persistent form of the TMA kernel
-  int ps_smem = 0, ps_ctas = 0, ps_stages = 0;
+  int ps_smem = 0, ps_ctas = 0, ps_stages = 0, ps_groups = 1;
   bool pdl = true;                        // programmatic dependent launch of the update kernel behind the schedule kernel
   bool fused_ok = false;                  // the single-launch path exists for this ctx (K, engine, variant)
   long long fused_max_tiles = 0;          // ... and is taken by launches of at most this many work items
@@ -256,8 +256,8 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     return bail(LAYUP_EINVAL);
   }
   ctx->engine = tune.engine == 2 ? 0 : 1;
-  ctx->variant = tune.variant;
   ctx->persistent = tune.launch_shape == 2;
+  ctx->variant = (ctx->persistent && tune.engine != 2) ? 0 : tune.variant;   // persistent TMA shape: variant = consumer groups
   ctx->pdl = tune.pdl != 2;
   if (ctx->engine == 1) {
     // TMA-staged kernel stages x, g (, m) of the whole tile: fall back to the LDG kernel if it does not fit
@@ -359,6 +359,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
       return bail(LAYUP_EINVAL);
     }
     ctx->ps_smem = (int)persist_smem_bytes(K, C, ctx->opt, ctx->ps_stages);
+    ctx->ps_groups = persist_groups(ctx->ps_stages, tune.variant);      // persistent shape: variant = consumer groups
     CU_TRY_INIT(persist_kernel_setup(ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->ps_smem, &ctx->ps_ctas));
     if (ctx->ps_ctas > want_ctas) ctx->ps_ctas = want_ctas;
     if (ctx->ps_ctas < 1) {
@@ -489,7 +490,7 @@ static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_
       // only the first update launch directly follows the schedule kernel on the stream
       if (ctx->ps_ok && !fused) {
         const int grid = (int)std::min<long long>(tab.prefix[n], (long long)ctx->n_sm * ctx->ps_ctas);
-        CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->ps_stages, ctx->pdl && n_launch == 0, s));
+        CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->ps_stages, ctx->ps_groups, ctx->pdl && n_launch == 0, s));
       } else {
         CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, fused, ctx->pdl && n_launch == 0, (int)tab.prefix[n], ctx->smem, s));
       }

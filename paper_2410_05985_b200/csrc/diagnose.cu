@@ -11,11 +11,12 @@
 //     memory ring with 1-D TMA bulk copies (cp.async.bulk, SASS UBLKCP), one copy per replica row
 //     spread over the warp's lanes, completing on the stage's "full" mbarrier; it re-arms a stage
 //     as soon as the stage's "empty" mbarrier has seen every consumer warp;
-//   * the CONSUMER warps never meet a CTA-wide barrier: a thread owns VEC scalar columns of the
-//     tile for ALL K replicas, so the consensus of its columns and the K squared distances are
-//     register arithmetic (fp64), with no exchange through shared memory.  For K <= 16 every
-//     element is converted to fp64 once and kept in registers for both passes, and the stage is
-//     released right after the loads; for larger K the second pass re-reads shared memory;
+//   * the CONSUMER warps (16 per CTA; 8 for K > 32, where the accumulators fill the register file)
+//     never meet a CTA-wide barrier: a thread owns ONE scalar column of the tile for ALL K replicas,
+//     so the consensus of its column and the K squared distances are register arithmetic (fp64),
+//     with no exchange through shared memory.  For K <= 16 every element is converted to fp64 once
+//     and kept in registers for both passes, and the stage is released right after the loads; for
+//     larger K the second pass re-reads shared memory;
 //   * a CTA walks a CONTIGUOUS range of the tile list, so it crosses a layer boundary only a few
 //     times; the per-replica partial sums stay in registers until then and leave through warp
 //     shuffles and one fp64 atomicAdd per (warp, replica).
@@ -26,9 +27,6 @@
 namespace layup {
 
 namespace {
-
-constexpr int kConsumers = 256;                 // consumer threads per CTA (8 warps)
-constexpr int kRingThreads = kConsumers + 32;   // + the producer warp
 
 struct DiagParams {
   const float *x;          // X section base
@@ -49,13 +47,14 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 // KT: compile-time bound on K (loops fully unrolled, accumulators in registers)
-// VEC: scalar columns per thread (tile row = kConsumers * VEC floats)
+// NCW: consumer warps; a thread owns ONE scalar column of the tile (tile row = NCW*32 floats)
 // KEEP: keep the converted tile in registers between the two passes (one fp32->fp64 conversion per element)
-template <int KT, int VEC, bool KEEP, int MINB>
-__global__ void __launch_bounds__(kRingThreads, MINB)
+template <int KT, bool KEEP, int NCW>
+__global__ void __launch_bounds__(NCW * 32 + 32, 1)
     layup_disagreement_kernel(const __grid_constant__ DiagParams p, const __grid_constant__ PosTable tab) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr int TF = kConsumers * VEC;                                   // floats per replica row of a tile
+  constexpr int NC = NCW * 32;                                           // consumer threads
+  constexpr int TF = NC;                                                 // floats per replica row of a tile
   const int K = p.K, S = p.stages, tid = threadIdx.x;
   float *ring = reinterpret_cast<float *>(smem_raw);                    // [S][K][TF]
   uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)S * K * TF);   // [S]
@@ -64,7 +63,7 @@ __global__ void __launch_bounds__(kRingThreads, MINB)
   if (tid == 0) {
     for (int s = 0; s < S; ++s) {
       mbar_init(full + s, 1);
-      mbar_init(empty + s, kConsumers / 32);
+      mbar_init(empty + s, NCW);
     }
   }
   __syncthreads();
@@ -83,9 +82,9 @@ __global__ void __launch_bounds__(kRingThreads, MINB)
     pos = lo;
   }
 
-  if (tid >= kConsumers) {
+  if (tid >= NC) {
     // ---------------- producer warp
-    const int lane = tid - kConsumers;
+    const int lane = tid - NC;
     int s = 0;
     uint32_t ph = 0;
     for (long long tile = t0; tile < t1; ++tile) {
@@ -105,7 +104,7 @@ __global__ void __launch_bounds__(kRingThreads, MINB)
     return;
   }
 
-  // ---------------- consumers: thread owns columns [VEC*tid, VEC*tid + VEC) for all K replicas
+  // ---------------- consumers: thread owns column `tid` of the tile for all K replicas
   // consensus coefficients: the scalar 1/K, or this layer's push-sum weights in a per-warp copy
   // (warps cross layer boundaries at different times and never synchronise with each other)
   double acc[KT];
@@ -117,7 +116,7 @@ __global__ void __launch_bounds__(kRingThreads, MINB)
   auto load_coef = [&](int q) {
     if (!weighted) return;
     __syncwarp();
-    for (int i = tid & 31; i < K; i += 32) coef[i] = __ldg(p.w + (size_t)tab.layer[q] * K + i);
+    for (int i = tid & 31; i < KT; i += 32) coef[i] = i < K ? __ldg(p.w + (size_t)tab.layer[q] * K + i) : 0.0;
     __syncwarp();
   };
   auto flush = [&](int q) {
@@ -140,62 +139,39 @@ __global__ void __launch_bounds__(kRingThreads, MINB)
       load_coef(pos);
     }
     const long long left = tab.lay[pos].pad - (tile - tab.prefix[pos]) * TF;
-    const bool live = (long long)(VEC * tid) < left;                    // pad % 32 == 0, VEC | 32: all or nothing
-    const float *row0 = ring + (size_t)s * K * TF + VEC * tid;
+    const float *row0 = ring + (size_t)s * K * TF + tid;
     mbar_wait(full + s, ph);
-    if (KEEP) {
-      double xd[KT][VEC], m[VEC];
-#pragma unroll
-      for (int v = 0; v < VEC; ++v) m[v] = 0.0;
+    if (KEEP && K == KT && left >= TF) {
+      // ---- whole tile, K == KT: no predicate anywhere; every element is converted once and kept in
+      // registers for both passes, the stage is released right after the loads, and the consensus
+      // sum runs on four chains
+      double xd[KT], m4[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
       for (int i = 0; i < KT; ++i) {
-        float xv[VEC];
-#pragma unroll
-        for (int v = 0; v < VEC; ++v) xv[v] = 0.f;
-        const double ci = weighted ? (i < K ? coef[i] : 0.0) : inv_k;
-        if (i < K && live) {
-          if (VEC == 2) { const float2 t = *reinterpret_cast<const float2 *>(row0 + (size_t)i * TF); xv[0] = t.x; xv[1] = t.y; }
-          else xv[0] = row0[(size_t)i * TF];
-        }
-#pragma unroll
-        for (int v = 0; v < VEC; ++v) {
-          xd[i][v] = (double)xv[v];
-          m[v] = fma(ci, xd[i][v], m[v]);
-        }
+        xd[i] = (double)row0[(size_t)i * TF];
+        m4[i & 3] = fma(weighted ? coef[i] : inv_k, xd[i], m4[i & 3]);
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(empty + s);                      // the tile now lives in registers
+      const double m = (m4[0] + m4[1]) + (m4[2] + m4[3]);
 #pragma unroll
       for (int i = 0; i < KT; ++i) {
-        if (i < K && live) {
-#pragma unroll
-          for (int v = 0; v < VEC; ++v) {
-            const double d = xd[i][v] - m[v];
-            acc[i] = fma(d, d, acc[i]);
-          }
-        }
+        const double d = xd[i] - m;
+        acc[i] = fma(d, d, acc[i]);
       }
     } else {
-      double m[VEC];
-#pragma unroll
-      for (int v = 0; v < VEC; ++v) m[v] = 0.0;
+      // ---- ragged tail of a layer, or K < KT: same arithmetic, predicated
+      const bool live = (long long)tid < left;                          // pads are part of the slice (zero in every replica)
+      double m = 0.0;
       if (live) {
 #pragma unroll
-        for (int i = 0; i < KT; ++i) {
-          if (i < K) {
-            const double ci = weighted ? coef[i] : inv_k;
-#pragma unroll
-            for (int v = 0; v < VEC; ++v) m[v] = fma(ci, (double)row0[(size_t)i * TF + v], m[v]);
-          }
-        }
+        for (int i = 0; i < KT; ++i)
+          if (i < K) m = fma(weighted ? coef[i] : inv_k, (double)row0[(size_t)i * TF], m);
 #pragma unroll
         for (int i = 0; i < KT; ++i) {
           if (i < K) {
-#pragma unroll
-            for (int v = 0; v < VEC; ++v) {
-              const double d = (double)row0[(size_t)i * TF + v] - m[v];
-              acc[i] = fma(d, d, acc[i]);
-            }
+            const double d = (double)row0[(size_t)i * TF] - m;
+            acc[i] = fma(d, d, acc[i]);
           }
         }
       }
@@ -331,16 +307,17 @@ __global__ void __launch_bounds__(kGenThreads) layup_disagreement_general(const 
 
 using DiagFn = void (*)(const DiagParams, const PosTable);
 struct RingShape {
-  int kt, vec, minb;
+  int kt, ncw;
   DiagFn fn;
 };
 // one CTA per SM: the registers go to the per-replica accumulators (and the fp64 copy of the tile),
-// the shared memory to a deep ring
+// the shared memory to a deep ring; 16 consumer warps while the accumulators allow it (8 were measured
+// issue-bound: profiles/r2_disagreement_gpt2m_k16_8warps.txt)
 const RingShape kRing[] = {
-    {8, 2, 1, layup_disagreement_kernel<8, 2, true, 1>},
-    {16, 2, 1, layup_disagreement_kernel<16, 2, true, 1>},
-    {32, 2, 1, layup_disagreement_kernel<32, 2, false, 1>},
-    {64, 1, 1, layup_disagreement_kernel<64, 1, false, 1>},
+    {8, 16, layup_disagreement_kernel<8, true, 16>},
+    {16, 16, layup_disagreement_kernel<16, true, 16>},
+    {32, 16, layup_disagreement_kernel<32, false, 16>},
+    {64, 8, layup_disagreement_kernel<64, false, 8>},
 };
 const RingShape *ring_shape(int K) {
   for (const RingShape &r : kRing)
@@ -348,8 +325,8 @@ const RingShape *ring_shape(int K) {
   return nullptr;
 }
 
-size_t ring_smem(int K, int tf, int stages, int kt) {
-  return (size_t)stages * K * tf * sizeof(float) + 16 * (size_t)stages + sizeof(double) * (kConsumers / 32) * (size_t)kt;
+size_t ring_smem(int K, int tf, int stages, int kt, int ncw) {
+  return (size_t)stages * K * tf * sizeof(float) + 16 * (size_t)stages + sizeof(double) * ncw * (size_t)kt;
 }
 size_t general_smem(int K, int C, bool two_stage) {
   return (two_stage ? 2 : 1) * (size_t)K * C * sizeof(float4) + sizeof(double) * (4 * (size_t)C + 2 * (size_t)K) + 16;
@@ -362,18 +339,18 @@ int general_iters(int K, int C) { return (K * C + kGenThreads - 1) / kGenThreads
 cudaError_t diag_plan(int K, size_t smem_optin, int *C, int *stages, int *smem_bytes, int *ctas_per_sm) {
   cudaError_t e;
   if (const RingShape *r = ring_shape(K)) {
-    const int tf = kConsumers * r->vec;
-    // as deep as fits: minb CTAs share ~224 KB of shared memory per SM
-    const size_t budget = (size_t)(224 * 1024) / r->minb - 1024 - sizeof(double) * (kConsumers / 32) * r->kt;
+    const int tf = r->ncw * 32;
+    // as deep as fits in the ~224 KB of shared memory of the SM's one CTA
+    const size_t budget = (size_t)(224 * 1024) - 1024 - sizeof(double) * r->ncw * r->kt;
     int S = (int)((budget < smem_optin ? budget : smem_optin) / ((size_t)K * tf * sizeof(float) + 16));
     if (S > 8) S = 8;
     if (S >= 2) {
       *C = tf / 4;
       *stages = S;
-      *smem_bytes = (int)ring_smem(K, tf, S, r->kt);
+      *smem_bytes = (int)ring_smem(K, tf, S, r->kt, r->ncw);
       if ((e = cudaFuncSetAttribute(r->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, *smem_bytes)) != cudaSuccess) return e;
       if ((e = cudaFuncSetAttribute(r->fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
-      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, r->fn, kRingThreads, *smem_bytes);
+      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, r->fn, r->ncw * 32 + 32, *smem_bytes);
     }
   }
   int c = 8;
@@ -392,8 +369,8 @@ cudaError_t launch_disagreement(const float *x, const double *w, double *dist, i
                                 const PosTable &tab, int grid, int smem_bytes, cudaStream_t s) {
   DiagParams p{x, w, dist, K, C, log2C, stages};
   const RingShape *r = ring_shape(K);
-  if (r && C * 4 == kConsumers * r->vec && stages >= 2 && (size_t)smem_bytes == ring_smem(K, C * 4, stages, r->kt)) {
-    r->fn<<<grid, kRingThreads, smem_bytes, s>>>(p, tab);
+  if (r && C * 4 == r->ncw * 32 && stages >= 2 && (size_t)smem_bytes == ring_smem(K, C * 4, stages, r->kt, r->ncw)) {
+    r->fn<<<grid, r->ncw * 32 + 32, smem_bytes, s>>>(p, tab);
     return cudaGetLastError();
   }
   if (general_iters(K, C) <= 8) layup_disagreement_general<8><<<grid, kGenThreads, smem_bytes, s>>>(p, tab);

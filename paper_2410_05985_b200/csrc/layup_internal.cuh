@@ -119,7 +119,8 @@ int persist_max_k();
 int persist_stages(int K, int C, int opt, size_t smem_optin, int ctas, int want);
 size_t persist_smem_bytes(int K, int C, int opt, int stages);
 cudaError_t persist_kernel_setup(int opt, bool symmetric, int smem_bytes, int *ctas_per_sm);
+int persist_groups(int stages, int want);
 cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, int grid, int smem_bytes, int stages,
-                                  bool pdl, cudaStream_t s);
+                                  int groups, bool pdl, cudaStream_t s);
 
 }  // namespace layup

@@ -4,8 +4,12 @@
 // frequent exactly there).  Same work item, same arithmetic (rule.cuh) and the same bits as
 // update_tma.cu.  Selected with layup_tuning.launch_shape = 2.
 //
-// Warp-specialised: every CTA is ONE producer warp plus kPsConsumers consumer threads around an
-// S-stage shared-memory ring (S >= 2, as deep as fits; layup_tuning.stages).
+// Warp-specialised: every CTA is ONE producer warp plus G consumer GROUPS of kPsGroup threads around
+// an S-stage shared-memory ring (S >= 2, as deep as fits; layup_tuning.stages).  The groups take the
+// CTA's tiles in turn (iteration n belongs to group n mod G), so G tiles are in different phases of
+// their computation at once -- what G resident CTAs give the grouped launch -- while the ring keeps
+// the next S-G tiles in flight (one group of 8 warps alone was measured issue-bound at 14 % of the
+// SM's warp slots: profiles/r2_update_persist_gpt2m_k16_1group.txt).
 //   producer  walks the CTA's share of the list (tile = blockIdx.x + n*gridDim.x, so the list is
 //             drained in order, output layer first); for each tile it waits for the stage's
 //             "empty" mbarrier, copies the layer's schedule tables (held in its registers, reloaded
@@ -14,8 +18,8 @@
 //             replica is active, else 1-D bulk copies of exactly the rows the flags ask for
 //             (an idle replica costs nothing, an idle receiver only its x row) -- the flags are in
 //             the producer's registers, so a straggler round's loads need no table round trip;
-//   consumers wait for "full", take the local steps out of shared memory (y overwrites x in place,
-//             m' / v' go to HBM), meet on a named barrier that only the consumer warps share, fold
+//   consumers (per group) wait for "full", take the local steps out of shared memory (y overwrites
+//             x in place, m' / v' go to HBM), meet on a named barrier that only the group shares, fold
 //             every receiver's senders and write x once, then release the stage ("empty").  No
 //             CTA-wide barrier exists, so the producer is never gated by the consumers' phases:
 //             up to S-1 tiles are in flight while one is computed.
@@ -27,15 +31,16 @@ namespace layup {
 
 namespace {
 
-constexpr int kPsConsumers = 256;
-constexpr int kPsThreads = kPsConsumers + 32;
+constexpr int kPsGroup = 256;                         // threads of one consumer group
+constexpr int kPsMaxGroups = 3;
+constexpr int kPsMaxThreads = kPsMaxGroups * kPsGroup + 32;
 constexpr int kPsMaxEntries = 4;                      // table entries per producer lane: K <= 128
 
 __device__ __forceinline__ void ps_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void consumer_barrier() {
-  asm volatile("bar.sync 1, %0;" ::"n"(kPsConsumers) : "memory");
+__device__ __forceinline__ void group_barrier(int group) {
+  asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(kPsGroup) : "memory");
 }
 
 // per-stage copy of a layer's schedule (what the consumers read)
@@ -58,12 +63,13 @@ __device__ __forceinline__ StageTables carve_tables(unsigned char *base, int K) 
 }
 
 template <int OPT, bool SYM>
-__global__ void __launch_bounds__(kPsThreads, 1)
+__global__ void __launch_bounds__(kPsMaxThreads, 1)
     layup_update_persist(const __grid_constant__ UpdateParams p, const __grid_constant__ PosTable tab, const int S) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int NARR = OptTraits<OPT>::kArrays;
   constexpr bool HAS_M = NARR >= 3, HAS_V = NARR >= 4;
-  const int K = p.K, C = p.C, log2C = p.log2C, tid = threadIdx.x;
+  const int K = p.K, C = p.C, log2C = p.log2C;
+  const int n_consumers = (int)blockDim.x - 32, G = n_consumers / kPsGroup;   // consumer groups
   const int n_items = K << log2C;
   const size_t stage_f4 = (size_t)NARR * n_items;                            // float4 per stage
   float4 *ring = reinterpret_cast<float4 *>(smem_raw);                       // [S][NARR][K*C]
@@ -72,19 +78,19 @@ __global__ void __launch_bounds__(kPsThreads, 1)
   unsigned char *tables0 = reinterpret_cast<unsigned char *>(empty + S);     // [S] StageTables
   const size_t tb = tables_bytes(K);
 
-  if (tid == 0) {
+  if (threadIdx.x == 0) {
     for (int s = 0; s < S; ++s) {
       mbar_init(full + s, 1);
-      mbar_init(empty + s, kPsConsumers / 32);
+      mbar_init(empty + s, kPsGroup / 32);              // a stage is consumed by one group
     }
   }
   __syncthreads();   // the only CTA-wide barrier: mbarriers visible
 
   const long long n_tiles = tab.prefix[tab.n];
 
-  if (tid >= kPsConsumers) {
+  if ((int)threadIdx.x >= n_consumers) {
     // ------------------------------------------------------------------ producer warp
-    const int lane = tid - kPsConsumers;
+    const int lane = (int)threadIdx.x - n_consumers;
     const bool boxed = p.all_active && p.tmaps != nullptr;
     int r_begin[kPsMaxEntries], r_cnt[kPsMaxEntries], r_send[kPsMaxEntries], r_flag[kPsMaxEntries];
     float r_alpha[kPsMaxEntries], r_c1[kPsMaxEntries], r_c2[kPsMaxEntries];
@@ -167,14 +173,21 @@ __global__ void __launch_bounds__(kPsThreads, 1)
     return;
   }
 
-  // -------------------------------------------------------------------- consumer warps
-  constexpr int NT = kPsConsumers;
-  int pos = 0, cur_pos = -1, s = 0;
-  uint32_t ph = 0;
-  for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+  // -------------------------------------------------------------------- consumer groups
+  constexpr int NT = kPsGroup;
+  const int group = (int)threadIdx.x / kPsGroup, tid = (int)threadIdx.x % kPsGroup;
+  int pos = 0, cur_pos = -1;
+  long long it = group;                                 // this group's iterations: group, group + G, ...
+  for (long long tile = blockIdx.x + it * gridDim.x; tile < n_tiles; tile += (long long)G * gridDim.x, it += G) {
+    const int s = (int)(it % S);
+    const uint32_t ph = (uint32_t)(it / S) & 1u;
     while (tile >= tab.prefix[pos + 1]) ++pos;
     if (pos != cur_pos) {
-      trace_start(p.trace, tab.layer[pos]);
+      if (p.trace != nullptr && tid == 0) {             // layup_trace: first start of the layer on this GPU
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        atomicMin(p.trace + tab.layer[pos], t);
+      }
       cur_pos = pos;
     }
     const long long pad = tab.lay[pos].pad;
@@ -203,12 +216,12 @@ __global__ void __launch_bounds__(kPsThreads, 1)
       if (HAS_V) st4(vb + off, v);
       xs[idx] = y;
     }
-    consumer_barrier();
+    group_barrier(group);
     if (SYM) {
       // ---- phase 2 (symmetric): every scalar column runs the K exchanges in worker order
       float *ysf = reinterpret_cast<float *>(xs);
       for (int e = tid; e < (ncols << 2); e += NT) symmetric_column(ysf, C << 2, e, K, T.senders);
-      consumer_barrier();
+      group_barrier(group);
       for (int idx = tid; idx < n_items; idx += NT) {
         const int i = idx >> log2C, c = idx & (C - 1);
         if (c >= ncols || !T.flags[i]) continue;          // idle and nobody's peer: 0 bytes
@@ -229,7 +242,6 @@ __global__ void __launch_bounds__(kPsThreads, 1)
     fence_proxy_async();   // the stage was written through the generic proxy; the TMA engine refills it next
     __syncwarp();
     if ((tid & 31) == 0) ps_arrive(empty + s);            // this warp is done with the stage
-    if (++s == S) { s = 0; ph ^= 1u; }
   }
 }
 
@@ -266,14 +278,21 @@ cudaError_t persist_kernel_setup(int opt, bool symmetric, int smem_bytes, int *c
   PsFn f = kPs[opt][symmetric ? 1 : 0];
   if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, f, kPsThreads, smem_bytes);
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, f, kPsMaxThreads, smem_bytes);
+}
+
+// Consumer groups for a ring of `stages`: leave at least one stage for the load in flight.
+int persist_groups(int stages, int want) {
+  int g = stages - 1 < kPsMaxGroups ? stages - 1 : kPsMaxGroups;
+  if (want > 0 && want < g) g = want;
+  return g < 1 ? 1 : g;
 }
 
 cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, int grid, int smem_bytes, int stages,
-                                  bool pdl, cudaStream_t s) {
+                                  int groups, bool pdl, cudaStream_t s) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
-  cfg.blockDim = dim3((unsigned)kPsThreads);
+  cfg.blockDim = dim3((unsigned)(groups * kPsGroup + 32));
   cfg.dynamicSmemBytes = (size_t)smem_bytes;
   cfg.stream = s;
   cudaLaunchAttribute attr[1];

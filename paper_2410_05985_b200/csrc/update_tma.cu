@@ -332,6 +332,7 @@ const TmaVariant kTma[] = {
     TmaVariant{128, 8, LAYUP_TMA_TABLE(false, 128, 8), LAYUP_TMA_NONE},
     TmaVariant{512, 2, LAYUP_TMA_TABLE(false, 512, 2), LAYUP_TMA_NONE},
     TmaVariant{256, 2, LAYUP_TMA_TABLE(false, 256, 2), LAYUP_TMA_NONE},
+    TmaVariant{512, 3, LAYUP_TMA_TABLE(false, 512, 3), LAYUP_TMA_NONE},
 };
 constexpr int kNumTma = sizeof(kTma) / sizeof(kTma[0]);
 
