@@ -89,6 +89,8 @@ typedef struct {
   int32_t tma2d;        /* 0 auto (by K and optimiser); 1: one 2-D tiled TMA load per
                            array and tile; 2: K 1-D bulk copies per array and tile                  */
   int32_t stages;       /* persistent shape: depth of the TMA ring; default: as deep as fits        */
+  int32_t group_threads;/* persistent shape: threads per consumer group (multiple of 32); default
+                           512 with one group, 256 with more                                        */
 } layup_tuning;
 
 typedef struct {

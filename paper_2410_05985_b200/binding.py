@@ -30,7 +30,7 @@ class LayUpError(RuntimeError):
 class _Tuning(ctypes.Structure):
     """layup_tuning of include/layup.h: 0 = the library's default in every field."""
     _fields_ = [(n, ctypes.c_int32) for n in ("engine", "launch_shape", "fused", "fused_waves", "tile_items", "variant",
-                                              "ctas_per_sm", "pdl", "tma2d", "stages")]
+                                              "ctas_per_sm", "pdl", "tma2d", "stages", "group_threads")]
 
 
 ENGINE_TMA, ENGINE_LDG = 1, 2

@@ -47,7 +47,7 @@ struct layup_ctx {
   int32_t *d_peer_scratch = nullptr, *d_ticket = nullptr;
   void *d_tmaps = nullptr;                // [n_sections][L] CUtensorMap: 2-D tiled view [K][pad] of every layer section
   bool ps_ok = false;                     // tuning.launch_shape == 2: persistent form of the TMA kernel
-  int ps_smem = 0, ps_ctas = 0, ps_stages = 0, ps_groups = 1;
+  int ps_smem = 0, ps_ctas = 0, ps_stages = 0, ps_groups = 1, ps_gs = 256;
   bool pdl = true;                        // programmatic dependent launch of the update kernel behind the schedule kernel
   bool fused_ok = false;                  // the single-launch path exists for this ctx (K, engine, variant)
   long long fused_max_tiles = 0;          // ... and is taken by launches of at most this many work items
@@ -145,7 +145,7 @@ static int check_config(const layup_config *cfg) {
     const layup_tuning &t = *cfg->tuning;
     if (t.engine < 0 || t.engine > 2 || t.launch_shape < 0 || t.launch_shape > 2 || t.fused < 0 || t.fused > 2 ||
         t.pdl < 0 || t.pdl > 2 || t.tma2d < 0 || t.tma2d > 2 || t.fused_waves < 0 || t.tile_items < 0 ||
-        t.variant < 0 || t.ctas_per_sm < 0 || t.stages < 0)
+        t.variant < 0 || t.ctas_per_sm < 0 || t.stages < 0 || t.group_threads < 0)
       return fail(nullptr, LAYUP_EINVAL, "layup_tuning field out of range");
   }
   return LAYUP_OK;
@@ -262,6 +262,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   if (ctx->engine == 1) {
     // TMA-staged kernel stages x, g (, m) of the whole tile: fall back to the LDG kernel if it does not fit
     if (ctx->variant < 0 || ctx->variant >= tma_num_variants()) ctx->variant = 0;
+    if (tune.variant == 0) ctx->variant = tma_default_variant(K * C, ctx->n_sections);
     ctx->fused_ok = K <= kFusedMaxK && tma_has_fused(ctx->variant) && tune.fused != 2;
     const size_t need_smem = tma_smem_bytes(K, C, ctx->opt, ctx->fused_ok);
     if (need_smem > prop.sharedMemPerBlockOptin) { ctx->engine = 0; ctx->fused_ok = false; }
@@ -315,7 +316,8 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   // 2-D tile loads replace K*arrays 1-D bulk copies per CTA by one per array.  Measured on B200: a
   // clear win without momentum (K = 16: 6.27 -> 6.94 TB/s) and from 64 copies per CTA up; at
   // K = 16 with momentum (48 copies) the 1-D form is 0.2 % ahead, so it is kept there.
-  const bool want_2d = tune.tma2d == 1 || (tune.tma2d == 0 && (ctx->n_sections == 2 || K * ctx->n_sections >= 64));
+  // (the persistent shape issues a tile's loads from one warp: always the 2-D form there)
+  const bool want_2d = tune.tma2d == 1 || (tune.tma2d == 0 && (ctx->n_sections == 2 || K * ctx->n_sections >= 64 || ctx->persistent));
   if (ctx->engine == 1 && want_2d && K <= 256 && C * 4 <= 256) {
     // One tensor map per (section, layer): rank 2, inner dim = the padded slice, outer dim = the K
     // replicas (stride = pad), box = [K][C*4 floats], no swizzle, zero fill past the slice end.
@@ -358,8 +360,8 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
       fail(nullptr, LAYUP_EINVAL, "launch_shape = persistent: two stages of this tile do not fit in shared memory");
       return bail(LAYUP_EINVAL);
     }
+    persist_shape(&ctx->ps_stages, K * C, tune.variant, tune.group_threads, &ctx->ps_groups, &ctx->ps_gs);
     ctx->ps_smem = (int)persist_smem_bytes(K, C, ctx->opt, ctx->ps_stages);
-    ctx->ps_groups = persist_groups(ctx->ps_stages, tune.variant);      // persistent shape: variant = consumer groups
     CU_TRY_INIT(persist_kernel_setup(ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->ps_smem, &ctx->ps_ctas));
     if (ctx->ps_ctas > want_ctas) ctx->ps_ctas = want_ctas;
     if (ctx->ps_ctas < 1) {
@@ -490,7 +492,7 @@ static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_
       // only the first update launch directly follows the schedule kernel on the stream
       if (ctx->ps_ok && !fused) {
         const int grid = (int)std::min<long long>(tab.prefix[n], (long long)ctx->n_sm * ctx->ps_ctas);
-        CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->ps_stages, ctx->ps_groups, ctx->pdl && n_launch == 0, s));
+        CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->ps_stages, ctx->ps_groups, ctx->ps_gs, ctx->pdl && n_launch == 0, s));
       } else {
         CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, fused, ctx->pdl && n_launch == 0, (int)tab.prefix[n], ctx->smem, s));
       }

@@ -7,7 +7,7 @@
 // 4 B of HBM traffic per parameter, so the roofline is the HBM read rate.
 //
 // Ring kernel (K <= 64), warp specialised:
-//   * one PRODUCER warp per CTA streams tiles (all K replicas x TF floats) into an S-stage shared
+//   * four PRODUCER warps per CTA stream tiles (all K replicas x TF floats) into an S-stage shared
 //     memory ring with 1-D TMA bulk copies (cp.async.bulk, SASS UBLKCP), one copy per replica row
 //     spread over the warp's lanes, completing on the stage's "full" mbarrier; it re-arms a stage
 //     as soon as the stage's "empty" mbarrier has seen every consumer warp;
@@ -48,9 +48,11 @@ __device__ __forceinline__ double warp_sum(double v) {
 
 // KT: compile-time bound on K (loops fully unrolled, accumulators in registers)
 // NCW: consumer warps; a thread owns ONE scalar column of the tile (tile row = NCW*32 floats)
+// kDiagProducers producer warps share a tile's row copies (a warp issues its bulk copies one lane at a time)
 // KEEP: keep the converted tile in registers between the two passes (one fp32->fp64 conversion per element)
+constexpr int kDiagProducers = 4;
 template <int KT, bool KEEP, int NCW>
-__global__ void __launch_bounds__(NCW * 32 + 32, 1)
+__global__ void __launch_bounds__(NCW * 32 + 32 * kDiagProducers, 1)
     layup_disagreement_kernel(const __grid_constant__ DiagParams p, const __grid_constant__ PosTable tab) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int NC = NCW * 32;                                           // consumer threads
@@ -68,7 +70,8 @@ __global__ void __launch_bounds__(NCW * 32 + 32, 1)
   }
   __syncthreads();
 
-  // contiguous share of the tile list
+  // contiguous share of the tile list (dealing the tiles round-robin over the CTAs was measured
+  // slower, 3.51 vs 3.19 ms on configs[2]: every CTA then crosses every layer boundary)
   const long long n_tiles = tab.prefix[tab.n];
   const long long t0 = n_tiles * blockIdx.x / gridDim.x, t1 = n_tiles * (blockIdx.x + 1) / gridDim.x;
   if (t0 >= t1) return;
@@ -83,8 +86,9 @@ __global__ void __launch_bounds__(NCW * 32 + 32, 1)
   }
 
   if (tid >= NC) {
-    // ---------------- producer warp
-    const int lane = tid - NC;
+    // ---------------- producer warps: row i of a tile goes to warp i mod kDiagProducers; warp 0 posts
+    // the stage's byte count (the only arrival "full" expects, so the phase cannot complete before it)
+    const int lane = (tid - NC) & 31, pw = (tid - NC) >> 5;
     int s = 0;
     uint32_t ph = 0;
     for (long long tile = t0; tile < t1; ++tile) {
@@ -95,10 +99,11 @@ __global__ void __launch_bounds__(NCW * 32 + 32, 1)
       const uint32_t chunk = (uint32_t)(left < TF ? left : TF) * 4u;     // multiple of 128 B
       const float *src = p.x + tab.lay[pos].base + f0;
       mbar_wait(empty + s, ph ^ 1u);                                    // the first pass over the ring is free
-      if (lane == 0) mbar_expect_tx(full + s, chunk * (uint32_t)K);
+      if (lane == 0 && pw == 0) mbar_expect_tx(full + s, chunk * (uint32_t)K);
       __syncwarp();
       float *dst = ring + (size_t)s * K * TF;
-      for (int i = lane; i < K; i += 32) bulk_g2s(dst + (size_t)i * TF, src + (long long)i * pad, chunk, full + s);
+      for (int i = pw + kDiagProducers * lane; i < K; i += 32 * kDiagProducers)
+        bulk_g2s(dst + (size_t)i * TF, src + (long long)i * pad, chunk, full + s);
       if (++s == S) { s = 0; ph ^= 1u; }
     }
     return;
@@ -350,7 +355,7 @@ cudaError_t diag_plan(int K, size_t smem_optin, int *C, int *stages, int *smem_b
       *smem_bytes = (int)ring_smem(K, tf, S, r->kt, r->ncw);
       if ((e = cudaFuncSetAttribute(r->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, *smem_bytes)) != cudaSuccess) return e;
       if ((e = cudaFuncSetAttribute(r->fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
-      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, r->fn, r->ncw * 32 + 32, *smem_bytes);
+      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, r->fn, r->ncw * 32 + 32 * kDiagProducers, *smem_bytes);
     }
   }
   int c = 8;
@@ -370,7 +375,7 @@ cudaError_t launch_disagreement(const float *x, const double *w, double *dist, i
   DiagParams p{x, w, dist, K, C, log2C, stages};
   const RingShape *r = ring_shape(K);
   if (r && C * 4 == r->ncw * 32 && stages >= 2 && (size_t)smem_bytes == ring_smem(K, C * 4, stages, r->kt, r->ncw)) {
-    r->fn<<<grid, r->ncw * 32 + 32, smem_bytes, s>>>(p, tab);
+    r->fn<<<grid, r->ncw * 32 + 32 * kDiagProducers, smem_bytes, s>>>(p, tab);
     return cudaGetLastError();
   }
   if (general_iters(K, C) <= 8) layup_disagreement_general<8><<<grid, kGenThreads, smem_bytes, s>>>(p, tab);

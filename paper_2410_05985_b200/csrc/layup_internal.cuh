@@ -108,6 +108,7 @@ cudaError_t launch_update(const UpdateParams &p, int variant, bool persistent, i
 size_t update_smem_bytes(int K, int C);
 // update_tma.cu -- TMA-bulk staged variants
 int tma_num_variants();
+int tma_default_variant(int n_items, int n_sections);
 size_t tma_smem_bytes(int K, int C, int opt, bool fused);
 bool tma_has_fused(int variant);
 cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_bytes, int *threads, int *ctas_per_sm);
@@ -119,8 +120,8 @@ int persist_max_k();
 int persist_stages(int K, int C, int opt, size_t smem_optin, int ctas, int want);
 size_t persist_smem_bytes(int K, int C, int opt, int stages);
 cudaError_t persist_kernel_setup(int opt, bool symmetric, int smem_bytes, int *ctas_per_sm);
-int persist_groups(int stages, int want);
+void persist_shape(int *stages, int n_items, int want_groups, int want_gs, int *groups, int *gs);
 cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, int grid, int smem_bytes, int stages,
-                                  int groups, bool pdl, cudaStream_t s);
+                                  int groups, int group_threads, bool pdl, cudaStream_t s);
 
 }  // namespace layup

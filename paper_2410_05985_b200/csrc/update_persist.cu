@@ -4,13 +4,16 @@
 // frequent exactly there).  Same work item, same arithmetic (rule.cuh) and the same bits as
 // update_tma.cu.  Selected with layup_tuning.launch_shape = 2.
 //
-// Warp-specialised: every CTA is ONE producer warp plus G consumer GROUPS of kPsGroup threads around
-// an S-stage shared-memory ring (S >= 2, as deep as fits; layup_tuning.stages).  The groups take the
-// CTA's tiles in turn (iteration n belongs to group n mod G), so G tiles are in different phases of
-// their computation at once -- what G resident CTAs give the grouped launch -- while the ring keeps
-// the next S-G tiles in flight (one group of 8 warps alone was measured issue-bound at 14 % of the
-// SM's warp slots: profiles/r2_update_persist_gpt2m_k16_1group.txt).
-//   producer  walks the CTA's share of the list (tile = blockIdx.x + n*gridDim.x, so the list is
+// Warp-specialised: every CTA is a few producer warps plus G consumer GROUPS of `gs` threads around
+// an S-stage shared-memory ring (S >= 2, as deep as fits; layup_tuning.stages, G divides S).  The
+// groups take the CTA's tiles in turn (iteration n uses stage n mod S and belongs to group n mod G),
+// so G tiles are in different phases of their computation at once -- what G resident CTAs give the
+// grouped launch -- while the ring keeps the next S-G tiles in flight (one group of 8 warps alone was
+// measured issue-bound at 14 % of the SM's warp slots: profiles/r2_update_persist_gpt2m_k16_1group.txt).
+// Because G divides S a stage is always consumed by the same group, so every waiter of an mbarrier
+// sees each of its phases (a group that skipped a phase would mistake an older completion of the
+// same parity for its own).
+//   producers walk the CTA's share of the list (tile = blockIdx.x + n*gridDim.x, so the list is
 //             drained in order, output layer first); for each tile it waits for the stage's
 //             "empty" mbarrier, copies the layer's schedule tables (held in its registers, reloaded
 //             only when the list crosses into another layer) into the stage, and issues the tile's
@@ -31,16 +34,16 @@ namespace layup {
 
 namespace {
 
-constexpr int kPsGroup = 256;                         // threads of one consumer group
-constexpr int kPsMaxGroups = 3;
-constexpr int kPsMaxThreads = kPsMaxGroups * kPsGroup + 32;
+constexpr int kPsProducers = 4;                       // producer warps (row copies are issued one lane at a time per warp)
+constexpr int kPsMaxConsumers = 768;                  // consumer threads per CTA, all groups together
+constexpr int kPsMaxThreads = kPsMaxConsumers + 32 * kPsProducers;
 constexpr int kPsMaxEntries = 4;                      // table entries per producer lane: K <= 128
 
 __device__ __forceinline__ void ps_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void group_barrier(int group) {
-  asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(kPsGroup) : "memory");
+__device__ __forceinline__ void group_barrier(int group, int threads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(threads) : "memory");
 }
 
 // per-stage copy of a layer's schedule (what the consumers read)
@@ -64,12 +67,13 @@ __device__ __forceinline__ StageTables carve_tables(unsigned char *base, int K) 
 
 template <int OPT, bool SYM>
 __global__ void __launch_bounds__(kPsMaxThreads, 1)
-    layup_update_persist(const __grid_constant__ UpdateParams p, const __grid_constant__ PosTable tab, const int S) {
+    layup_update_persist(const __grid_constant__ UpdateParams p, const __grid_constant__ PosTable tab, const int S,
+                         const int G) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int NARR = OptTraits<OPT>::kArrays;
   constexpr bool HAS_M = NARR >= 3, HAS_V = NARR >= 4;
   const int K = p.K, C = p.C, log2C = p.log2C;
-  const int n_consumers = (int)blockDim.x - 32, G = n_consumers / kPsGroup;   // consumer groups
+  const int n_consumers = (int)blockDim.x - 32 * kPsProducers, gthreads = n_consumers / G;   // threads per consumer group
   const int n_items = K << log2C;
   const size_t stage_f4 = (size_t)NARR * n_items;                            // float4 per stage
   float4 *ring = reinterpret_cast<float4 *>(smem_raw);                       // [S][NARR][K*C]
@@ -81,7 +85,7 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
   if (threadIdx.x == 0) {
     for (int s = 0; s < S; ++s) {
       mbar_init(full + s, 1);
-      mbar_init(empty + s, kPsGroup / 32);              // a stage is consumed by one group
+      mbar_init(empty + s, gthreads / 32);                    // a stage is consumed by one group
     }
   }
   __syncthreads();   // the only CTA-wide barrier: mbarriers visible
@@ -89,9 +93,10 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
   const long long n_tiles = tab.prefix[tab.n];
 
   if ((int)threadIdx.x >= n_consumers) {
-    // ------------------------------------------------------------------ producer warp
-    const int lane = (int)threadIdx.x - n_consumers;
+    // ------------------------------------------------------------------ producer warps
+    const int lane = ((int)threadIdx.x - n_consumers) & 31, pw = ((int)threadIdx.x - n_consumers) >> 5;
     const bool boxed = p.all_active && p.tmaps != nullptr;
+    if (boxed && pw >= NARR) return;                    // whole-tile 2-D loads: one producer warp per array
     int r_begin[kPsMaxEntries], r_cnt[kPsMaxEntries], r_send[kPsMaxEntries], r_flag[kPsMaxEntries];
     float r_alpha[kPsMaxEntries], r_c1[kPsMaxEntries], r_c2[kPsMaxEntries];
     int pos = 0, cur_pos = -1, s = 0;
@@ -126,13 +131,13 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
       const uint32_t chunk = (uint32_t)(cols_left < C ? cols_left : C) * 16u;
 
       mbar_wait(empty + s, ph ^ 1u);                      // the first trip round the ring is free
-      // hand the layer's tables to the consumers through the stage
+      // producer warp 0 hands the layer's tables to the consumers through the stage
       const StageTables T = carve_tables(tables0 + (size_t)s * tb, K);
       uint32_t bytes = 0;
 #pragma unroll
       for (int e = 0; e < kPsMaxEntries; ++e) {
         const int k = lane + 32 * e;
-        if (k < K) {
+        if (k < K && pw == 0) {
           T.begin[k] = r_begin[e]; T.cnt[k] = r_cnt[e]; T.senders[k] = r_send[e]; T.alpha[k] = r_alpha[e];
           if (HAS_V) { T.c1[k] = r_c1[e]; T.c2[k] = r_c2[e]; }
           T.flags[k] = (unsigned char)r_flag[e];
@@ -141,19 +146,25 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
       }
       float4 *st = ring + (size_t)s * stage_f4;
       if (boxed) {
+        // one 2-D tiled load per array, array a from producer warp a: a tensor load keeps its issuing
+        // thread busy for some hundred ns (measured: ~2 us per tile when one thread issued all three),
+        // so the arrays go out side by side.  Warp 0 posts the byte count of the whole stage -- the
+        // only arrival the "full" barrier expects, so the phase cannot complete before it.
         __syncwarp();                                     // table stores of all lanes before lane 0's arrive (release)
         if (lane == 0) {
-          mbar_expect_tx(full + s, (uint32_t)n_items * 16u * NARR);
+          if (pw == 0) mbar_expect_tx(full + s, (uint32_t)n_items * 16u * NARR);
           const unsigned char *tm = reinterpret_cast<const unsigned char *>(p.tmaps);
-#pragma unroll
-          for (int a = 0; a < NARR; ++a)
-            tma_load_2d(st + a * n_items, tm + ((size_t)a * p.L + tab.layer[pos]) * 128, (int)(col0 << 2), 0, full + s);
+          tma_load_2d(st + pw * n_items, tm + ((size_t)pw * p.L + tab.layer[pos]) * 128, (int)(col0 << 2), 0, full + s);
         }
       } else {
+        // Row copies: warp 0 posts the stage's byte count (the only arrival the "full" barrier expects,
+        // so the phase cannot complete before it, whatever the other warps' copies have already
+        // delivered); array a of every row goes to producer warp a mod kPsProducers -- a warp issues
+        // its bulk copies one lane at a time, four warps keep the TMA unit fed.
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xFFFFFFFFu, bytes, o);
         __syncwarp();
-        if (lane == 0) mbar_expect_tx(full + s, bytes);
+        if (lane == 0 && pw == 0) mbar_expect_tx(full + s, bytes);
         __syncwarp();
         const long long tile_off = tab.lay[pos].base + (col0 << 2);
 #pragma unroll
@@ -162,6 +173,7 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
           if (i < K && r_flag[e]) {
             const int na = (r_flag[e] & kFlagActive) ? NARR : 1;
             for (int a = 0; a < na; ++a) {
+              if (((a + i) & (kPsProducers - 1)) != pw) continue;
               const float *src = (a == 0 ? p.x : a == 1 ? p.g : a == 2 ? p.m : p.v) + tile_off + (long long)i * pad;
               bulk_g2s(st + a * n_items + (i << log2C), src, chunk, full + s);
             }
@@ -174,8 +186,8 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
   }
 
   // -------------------------------------------------------------------- consumer groups
-  constexpr int NT = kPsGroup;
-  const int group = (int)threadIdx.x / kPsGroup, tid = (int)threadIdx.x % kPsGroup;
+  const int NT = gthreads;
+  const int group = (int)threadIdx.x / gthreads, tid = (int)threadIdx.x % gthreads;
   int pos = 0, cur_pos = -1;
   long long it = group;                                 // this group's iterations: group, group + G, ...
   for (long long tile = blockIdx.x + it * gridDim.x; tile < n_tiles; tile += (long long)G * gridDim.x, it += G) {
@@ -216,12 +228,12 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
       if (HAS_V) st4(vb + off, v);
       xs[idx] = y;
     }
-    group_barrier(group);
+    group_barrier(group, gthreads);
     if (SYM) {
       // ---- phase 2 (symmetric): every scalar column runs the K exchanges in worker order
       float *ysf = reinterpret_cast<float *>(xs);
       for (int e = tid; e < (ncols << 2); e += NT) symmetric_column(ysf, C << 2, e, K, T.senders);
-      group_barrier(group);
+      group_barrier(group, gthreads);
       for (int idx = tid; idx < n_items; idx += NT) {
         const int i = idx >> log2C, c = idx & (C - 1);
         if (c >= ncols || !T.flags[i]) continue;          // idle and nobody's peer: 0 bytes
@@ -245,7 +257,7 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
   }
 }
 
-using PsFn = void (*)(const UpdateParams, const PosTable, const int);
+using PsFn = void (*)(const UpdateParams, const PosTable, const int, const int);
 const PsFn kPs[3][2] = {{layup_update_persist<OPT_SGD, false>, layup_update_persist<OPT_SGD, true>},
                         {layup_update_persist<OPT_SGD_MOM, false>, layup_update_persist<OPT_SGD_MOM, true>},
                         {layup_update_persist<OPT_ADAMW, false>, layup_update_persist<OPT_ADAMW, true>}};
@@ -281,18 +293,27 @@ cudaError_t persist_kernel_setup(int opt, bool symmetric, int smem_bytes, int *c
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, f, kPsMaxThreads, smem_bytes);
 }
 
-// Consumer groups for a ring of `stages`: leave at least one stage for the load in flight.
-int persist_groups(int stages, int want) {
-  int g = stages - 1 < kPsMaxGroups ? stages - 1 : kPsMaxGroups;
-  if (want > 0 && want < g) g = want;
-  return g < 1 ? 1 : g;
+// Shape of the consumer side for a ring of *stages and a tile of `n_items` float4 items: G groups of
+// gs threads.  G divides the ring depth (the depth is trimmed to a multiple of G) and every group
+// keeps at least two stages, one computing and one in flight; gs is a multiple of 32, at most the
+// tile, and G*gs <= kPsMaxConsumers.  want_groups / want_gs > 0: the caller's choice, made legal.
+void persist_shape(int *stages, int n_items, int want_groups, int want_gs, int *groups, int *gs) {
+  int g = want_groups > 0 ? want_groups : (*stages >= 4 ? 2 : 1);
+  while (g > 1 && *stages / g < 2) --g;
+  *stages -= *stages % g;
+  int t = want_gs > 0 ? want_gs : (g == 1 ? 512 : 256);
+  t = t / 32 * 32;
+  if (t < 32) t = 32;
+  while (t > 32 && (t * g > kPsMaxConsumers || t > n_items)) t -= 32;
+  *groups = g;
+  *gs = t;
 }
 
 cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, int grid, int smem_bytes, int stages,
-                                  int groups, bool pdl, cudaStream_t s) {
+                                  int groups, int group_threads, bool pdl, cudaStream_t s) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
-  cfg.blockDim = dim3((unsigned)(groups * kPsGroup + 32));
+  cfg.blockDim = dim3((unsigned)(groups * group_threads + 32 * kPsProducers));
   cfg.dynamicSmemBytes = (size_t)smem_bytes;
   cfg.stream = s;
   cudaLaunchAttribute attr[1];
@@ -300,7 +321,7 @@ cudaError_t launch_update_persist(const UpdateParams &p, const PosTable &tab, in
   attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, kPs[p.opt][p.symmetric ? 1 : 0], p, tab, stages);
+  return cudaLaunchKernelEx(&cfg, kPs[p.opt][p.symmetric ? 1 : 0], p, tab, stages, groups);
 }
 
 }  // namespace layup

@@ -47,7 +47,7 @@ def test_tuning_block_is_the_only_switch(lib):
     text = open(os.path.join(ROOT, "include", "layup.h")).read()
     body = re.search(r"typedef struct \{(.*?)\} layup_tuning;", text, flags=re.S).group(1)
     fields = re.findall(r"int32_t\s+(\w+)\s*;\s*/\*", body)               # name followed by its comment
-    assert fields == [f[0] for f in binding._Tuning._fields_] and len(fields) == 10
+    assert fields == [f[0] for f in binding._Tuning._fields_] and len(fields) == 11
     for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2410_05985_b200")):
         for f in files:
             if f.endswith((".cu", ".cuh", ".h", ".py")):
