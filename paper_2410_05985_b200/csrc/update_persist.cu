@@ -22,10 +22,10 @@
 //             (an idle replica costs nothing, an idle receiver only its x row) -- the flags are in
 //             the producer's registers, so a straggler round's loads need no table round trip;
 //   consumers (per group) wait for "full", take the local steps out of shared memory (y overwrites
-//             x in place, m' / v' go to HBM), meet on a named barrier that only the group shares, fold
-//             every receiver's senders and write x once, then release the stage ("empty").  No
-//             CTA-wide barrier exists, so the producer is never gated by the consumers' phases:
-//             up to S-1 tiles are in flight while one is computed.
+//             x in place, m' / v' go to HBM), meet on a named barrier that only the group shares,
+//             hand the g / m / v slots of the stage back ("empty" per array: they are refilled while
+//             the mix runs), fold every receiver's senders, write x once and release the x slot.
+//             No CTA-wide barrier exists, so the producers are never gated by the consumers' phases.
 #include "layup_internal.cuh"
 #include "rule.cuh"
 #include "tma_ptx.cuh"
@@ -77,15 +77,17 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
   const int n_items = K << log2C;
   const size_t stage_f4 = (size_t)NARR * n_items;                            // float4 per stage
   float4 *ring = reinterpret_cast<float4 *>(smem_raw);                       // [S][NARR][K*C]
-  uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)S * stage_f4);    // [S]
-  uint64_t *empty = full + S;                                                // [S]
-  unsigned char *tables0 = reinterpret_cast<unsigned char *>(empty + S);     // [S] StageTables
+  // one full/empty pair per (stage, array): the g / m / v slots of a stage are handed back to the
+  // producers right after the local step, only the x slot (it holds y) lives through the mix
+  uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)S * stage_f4);    // [S][NARR]
+  uint64_t *empty = full + S * NARR;                                         // [S][NARR]
+  unsigned char *tables0 = reinterpret_cast<unsigned char *>(empty + S * NARR);   // [S] StageTables
   const size_t tb = tables_bytes(K);
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < S; ++s) {
+    for (int s = 0; s < S * NARR; ++s) {
       mbar_init(full + s, 1);
-      mbar_init(empty + s, gthreads / 32);                    // a stage is consumed by one group
+      mbar_init(empty + s, gthreads / 32);                // a stage is consumed by one group
     }
   }
   __syncthreads();   // the only CTA-wide barrier: mbarriers visible
@@ -94,13 +96,18 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
 
   if ((int)threadIdx.x >= n_consumers) {
     // ------------------------------------------------------------------ producer warps
+    // warp pw feeds array a = pw mod NARR; with two arrays the rows of a straggler round are split
+    // between two warps per array (a warp issues its bulk copies one lane at a time, ~22 per us)
+    constexpr int R = kPsProducers / NARR;              // warps per array: 2, 1, 1 for 2, 3, 4 arrays
     const int lane = ((int)threadIdx.x - n_consumers) & 31, pw = ((int)threadIdx.x - n_consumers) >> 5;
+    const int a = pw % NARR, r = pw / NARR;
     const bool boxed = p.all_active && p.tmaps != nullptr;
-    if (boxed && pw >= NARR) return;                    // whole-tile 2-D loads: one producer warp per array
+    if (r >= R || (boxed && r > 0)) return;             // spare warp; whole-tile 2-D loads need one warp per array
     int r_begin[kPsMaxEntries], r_cnt[kPsMaxEntries], r_send[kPsMaxEntries], r_flag[kPsMaxEntries];
     float r_alpha[kPsMaxEntries], r_c1[kPsMaxEntries], r_c2[kPsMaxEntries];
     int pos = 0, cur_pos = -1, s = 0;
     uint32_t ph = 0;
+    const float *const asrc = a == 0 ? p.x : a == 1 ? p.g : a == 2 ? p.m : p.v;
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
       while (tile >= tab.prefix[pos + 1]) ++pos;
       if (pos != cur_pos) {
@@ -113,14 +120,16 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
           const int k = lane + 32 * e;
           r_flag[e] = 0;
           if (k < K) {
-            r_send[e] = SYM ? p.t.peer[row + k] : p.t.senders[row + k];
-            r_alpha[e] = p.t.alpha[row + k];
             r_flag[e] = p.t.flags[row + k];
-            const int b = p.t.recv_off[(size_t)layer * (K + 1) + k];
-            r_begin[e] = b;
-            r_cnt[e] = p.t.recv_off[(size_t)layer * (K + 1) + k + 1] - b;
-            r_c1[e] = HAS_V ? p.t.c1[row + k] : 0.f;
-            r_c2[e] = HAS_V ? p.t.c2[row + k] : 0.f;
+            if (pw == 0) {                                // only the x warp passes the tables on
+              r_send[e] = SYM ? p.t.peer[row + k] : p.t.senders[row + k];
+              r_alpha[e] = p.t.alpha[row + k];
+              const int b = p.t.recv_off[(size_t)layer * (K + 1) + k];
+              r_begin[e] = b;
+              r_cnt[e] = p.t.recv_off[(size_t)layer * (K + 1) + k + 1] - b;
+              r_c1[e] = HAS_V ? p.t.c1[row + k] : 0.f;
+              r_c2[e] = HAS_V ? p.t.c2[row + k] : 0.f;
+            }
           }
         }
         cur_pos = pos;
@@ -129,55 +138,51 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
       const long long col0 = (tile - tab.prefix[pos]) << log2C;
       const long long cols_left = (pad >> 2) - col0;
       const uint32_t chunk = (uint32_t)(cols_left < C ? cols_left : C) * 16u;
+      uint64_t *const fbar = full + s * NARR + a;
 
-      mbar_wait(empty + s, ph ^ 1u);                      // the first trip round the ring is free
-      // producer warp 0 hands the layer's tables to the consumers through the stage
-      const StageTables T = carve_tables(tables0 + (size_t)s * tb, K);
-      uint32_t bytes = 0;
+      mbar_wait(empty + s * NARR + a, ph ^ 1u);           // the first trip round the ring is free
+      if (pw == 0) {
+        // hand the layer's tables to the consumers through the stage (they acquire them with the x slot)
+        const StageTables T = carve_tables(tables0 + (size_t)s * tb, K);
 #pragma unroll
-      for (int e = 0; e < kPsMaxEntries; ++e) {
-        const int k = lane + 32 * e;
-        if (k < K && pw == 0) {
-          T.begin[k] = r_begin[e]; T.cnt[k] = r_cnt[e]; T.senders[k] = r_send[e]; T.alpha[k] = r_alpha[e];
-          if (HAS_V) { T.c1[k] = r_c1[e]; T.c2[k] = r_c2[e]; }
-          T.flags[k] = (unsigned char)r_flag[e];
-          bytes += r_flag[e] ? chunk * ((r_flag[e] & kFlagActive) ? (uint32_t)NARR : 1u) : 0u;
+        for (int e = 0; e < kPsMaxEntries; ++e) {
+          const int k = lane + 32 * e;
+          if (k < K) {
+            T.begin[k] = r_begin[e]; T.cnt[k] = r_cnt[e]; T.senders[k] = r_send[e]; T.alpha[k] = r_alpha[e];
+            if (HAS_V) { T.c1[k] = r_c1[e]; T.c2[k] = r_c2[e]; }
+            T.flags[k] = (unsigned char)r_flag[e];
+          }
         }
       }
-      float4 *st = ring + (size_t)s * stage_f4;
+      float4 *dst = ring + (size_t)s * stage_f4 + (size_t)a * n_items;
       if (boxed) {
-        // one 2-D tiled load per array, array a from producer warp a: a tensor load keeps its issuing
-        // thread busy for some hundred ns (measured: ~2 us per tile when one thread issued all three),
-        // so the arrays go out side by side.  Warp 0 posts the byte count of the whole stage -- the
-        // only arrival the "full" barrier expects, so the phase cannot complete before it.
+        // ONE 2-D tiled load for this array's tile; the arrays go out side by side from their warps
         __syncwarp();                                     // table stores of all lanes before lane 0's arrive (release)
         if (lane == 0) {
-          if (pw == 0) mbar_expect_tx(full + s, (uint32_t)n_items * 16u * NARR);
+          mbar_expect_tx(fbar, (uint32_t)n_items * 16u);
           const unsigned char *tm = reinterpret_cast<const unsigned char *>(p.tmaps);
-          tma_load_2d(st + pw * n_items, tm + ((size_t)pw * p.L + tab.layer[pos]) * 128, (int)(col0 << 2), 0, full + s);
+          tma_load_2d(dst, tm + ((size_t)a * p.L + tab.layer[pos]) * 128, (int)(col0 << 2), 0, fbar);
         }
       } else {
-        // Row copies: warp 0 posts the stage's byte count (the only arrival the "full" barrier expects,
-        // so the phase cannot complete before it, whatever the other warps' copies have already
-        // delivered); array a of every row goes to producer warp a mod kPsProducers -- a warp issues
-        // its bulk copies one lane at a time, four warps keep the TMA unit fed.
+        // Row copies of exactly the rows the flags ask for: x for every replica that is active or
+        // receives, g / m / v for the active ones.  Warp r == 0 of the array posts the byte count --
+        // the only arrival the slot's "full" barrier expects, so the phase cannot complete before
+        // it, whatever the other warp's copies have already delivered.
+        uint32_t bytes = 0;
+#pragma unroll
+        for (int e = 0; e < kPsMaxEntries; ++e)
+          if (lane + 32 * e < K && (a == 0 ? r_flag[e] != 0 : (r_flag[e] & kFlagActive) != 0)) bytes += chunk;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xFFFFFFFFu, bytes, o);
         __syncwarp();
-        if (lane == 0 && pw == 0) mbar_expect_tx(full + s, bytes);
+        if (lane == 0 && r == 0) mbar_expect_tx(fbar, bytes);
         __syncwarp();
         const long long tile_off = tab.lay[pos].base + (col0 << 2);
 #pragma unroll
         for (int e = 0; e < kPsMaxEntries; ++e) {
           const int i = lane + 32 * e;
-          if (i < K && r_flag[e]) {
-            const int na = (r_flag[e] & kFlagActive) ? NARR : 1;
-            for (int a = 0; a < na; ++a) {
-              if (((a + i) & (kPsProducers - 1)) != pw) continue;
-              const float *src = (a == 0 ? p.x : a == 1 ? p.g : a == 2 ? p.m : p.v) + tile_off + (long long)i * pad;
-              bulk_g2s(st + a * n_items + (i << log2C), src, chunk, full + s);
-            }
-          }
+          if (i < K && (i % R) == r && (a == 0 ? r_flag[e] != 0 : (r_flag[e] & kFlagActive) != 0))
+            bulk_g2s(dst + (i << log2C), asrc + tile_off + (long long)i * pad, chunk, fbar);
         }
       }
       if (++s == S) { s = 0; ph ^= 1u; }
@@ -213,7 +218,8 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
     float4 *xs = ring + (size_t)s * stage_f4, *gs = xs + n_items;
     float4 *ms = HAS_M ? gs + n_items : gs, *vs = HAS_V ? ms + n_items : ms;
     const StageTables T = carve_tables(tables0 + (size_t)s * tb, K);
-    mbar_wait(full + s, ph);                              // tile and tables have landed (acquire)
+#pragma unroll
+    for (int a = 0; a < NARR; ++a) mbar_wait(full + s * NARR + a, ph);   // tile and tables have landed (acquire)
 
     // ---- phase 1: local step; y overwrites x in place, m' (v') -> HBM
     for (int idx = tid; idx < n_items; idx += NT) {
@@ -229,6 +235,11 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
       xs[idx] = y;
     }
     group_barrier(group, gthreads);
+    // every thread of the group is past its reads of g, m, v: those slots go back to the producers now
+    if ((tid & 31) == 0) {
+#pragma unroll
+      for (int a = 1; a < NARR; ++a) ps_arrive(empty + s * NARR + a);
+    }
     if (SYM) {
       // ---- phase 2 (symmetric): every scalar column runs the K exchanges in worker order
       float *ysf = reinterpret_cast<float *>(xs);
@@ -251,9 +262,9 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
         st4(xb + (long long)i * pad + (c << 2), acc);
       }
     }
-    fence_proxy_async();   // the stage was written through the generic proxy; the TMA engine refills it next
+    fence_proxy_async();   // the x slot was written through the generic proxy; the TMA engine refills it next
     __syncwarp();
-    if ((tid & 31) == 0) ps_arrive(empty + s);            // this warp is done with the stage
+    if ((tid & 31) == 0) ps_arrive(empty + s * NARR);     // this warp is done with the stage
   }
 }
 
@@ -264,7 +275,7 @@ const PsFn kPs[3][2] = {{layup_update_persist<OPT_SGD, false>, layup_update_pers
 
 size_t stage_bytes(int K, int C, int opt) {
   const int narr = opt == OPT_ADAMW ? 4 : opt == OPT_SGD_MOM ? 3 : 2;
-  return (size_t)K * C * sizeof(float4) * narr + 16 + tables_bytes(K);
+  return (size_t)K * C * sizeof(float4) * narr + 16 * (size_t)narr + tables_bytes(K);   // arrays, mbarrier pairs, tables
 }
 
 }  // namespace

@@ -1,10 +1,11 @@
 """Turn ncu captures of the library's kernels into the text summaries kept under profiles/.
 
-  python -m paper_2410_05985_b200.ncu_summary traffic  REP:WORKLOAD:OPTIMIZER [...]  > profiles/traffic.csv
+  python -m paper_2410_05985_b200.ncu_summary traffic  REP:WORKLOAD:OPTIMIZER[:KERNEL_REGEX[:SUMMARY]] [...]  > profiles/traffic.csv
   python -m paper_2410_05985_b200.ncu_summary summary  REP [KERNEL_REGEX]            > profiles/<name>.txt
 
 `traffic` writes one csv row per capture: dram__bytes_read.sum + dram__bytes_write.sum of the
-(last) matching kernel launch in REP, i.e. the number bench.py reports as roofline.traffic.
+(last) matching kernel launch in REP, i.e. the number bench.py reports as roofline.traffic
+(SUMMARY: the committed text summary of the same capture, written to the `source` column).
 `summary` prints the counters DESIGN.md quotes (duration, DRAM bytes and throughput, occupancy,
 registers, issue utilisation, top stall reasons) for every matching launch.
 Both read the report with `ncu -i REP --page raw --csv`; nothing here runs on a GPU.
@@ -48,11 +49,13 @@ def traffic(specs):
     w = csv.writer(sys.stdout, lineterminator="\n")
     w.writerow(["workload", "optimizer", "dram_bytes_per_launch", "kernel", "source"])
     for spec in specs:
-        rep, workload, optimizer = spec.split(":")[:3]
-        pattern = spec.split(":")[3] if spec.count(":") >= 3 else r"layup_update"
+        parts = spec.split(":")
+        rep, workload, optimizer = parts[:3]
+        pattern = parts[3] if len(parts) > 3 and parts[3] else r"layup_update"
+        source = parts[4] if len(parts) > 4 else rep
         l = pick(read_raw(rep), pattern)[-1]
         total = scaled(l, "dram__bytes_read.sum") + scaled(l, "dram__bytes_write.sum")
-        w.writerow([workload, optimizer, int(round(total)), kernel_short(l["Kernel Name"][0]), rep])
+        w.writerow([workload, optimizer, int(round(total)), kernel_short(l["Kernel Name"][0]), source])
 
 
 _SUMMARY = ["gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum",
