@@ -53,6 +53,8 @@ struct layup_ctx {
   long long fused_max_tiles = 0;          // ... and is taken by launches of at most this many work items
   unsigned char *d_active_scratch = nullptr;
   uint32_t *d_step = nullptr;             // [L] round each layer runs next (device state, see layup.h graphs)
+  int32_t *d_ps_ticket = nullptr;         // [n_ps_ticket] tile tickets of persistent update launches
+  int n_ps_ticket = 0;
   unsigned long long *d_trace = nullptr;  // [L] layup_trace
   bool tracing = false;
   // bookkeeping
@@ -310,6 +312,9 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   CU_TRY_INIT(cudaMalloc(&ctx->d_dist, sizeof(double) * L * K));
   CU_TRY_INIT(cudaMalloc(&ctx->d_step, sizeof(uint32_t) * L));
   CU_TRY_INIT(cudaMemset(ctx->d_step, 0, sizeof(uint32_t) * L));
+  ctx->n_ps_ticket = (L + kMaxPos - 1) / kMaxPos + 8;
+  CU_TRY_INIT(cudaMalloc(&ctx->d_ps_ticket, sizeof(int32_t) * ctx->n_ps_ticket));
+  CU_TRY_INIT(cudaMemset(ctx->d_ps_ticket, 0, sizeof(int32_t) * ctx->n_ps_ticket));
   CU_TRY_INIT(cudaMalloc(&ctx->d_trace, sizeof(unsigned long long) * L));
   CU_TRY_INIT(cudaMemset(ctx->d_trace, 0xFF, sizeof(unsigned long long) * L));
   ctx->last_event_step.assign(L, -1);
@@ -408,7 +413,7 @@ extern "C" int layup_destroy(layup_ctx *ctx) {
   cudaFree(ctx->t.peer); cudaFree(ctx->t.recv_off); cudaFree(ctx->t.senders); cudaFree(ctx->t.alpha);
   cudaFree(ctx->t.c1); cudaFree(ctx->t.c2); cudaFree(ctx->d_bpow);
   cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_ticket); cudaFree(ctx->d_tmaps);
-  cudaFree(ctx->d_active_scratch); cudaFree(ctx->d_dist); cudaFree(ctx->d_step); cudaFree(ctx->d_trace);
+  cudaFree(ctx->d_active_scratch); cudaFree(ctx->d_dist); cudaFree(ctx->d_step); cudaFree(ctx->d_trace); cudaFree(ctx->d_ps_ticket);
   delete ctx;
   return LAYUP_OK;
 }
@@ -450,6 +455,7 @@ static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_
   sp.mix_mode = ctx->mix_mode; sp.adamw = ctx->opt == OPT_ADAMW ? 1 : 0; sp.bpow = ctx->d_bpow;
   sp.lr = (double)ctx->lr; sp.beta1 = (double)ctx->beta1; sp.beta2 = (double)ctx->beta2;
   sp.ticket = ctx->d_ticket;
+  sp.ps_ticket = ctx->d_ps_ticket; sp.n_ps_ticket = ctx->ps_ok ? ctx->n_ps_ticket : 0;
   const bool fused = ctx->fused_ok && ctx->tile_prefix[pos_end] - ctx->tile_prefix[pos_begin] <= ctx->fused_max_tiles;
   if (!fused) CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
 
@@ -491,6 +497,8 @@ static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_
       tab.n = n;
       // only the first update launch directly follows the schedule kernel on the stream
       if (ctx->ps_ok && !fused) {
+        if (n_launch >= ctx->n_ps_ticket) return fail(ctx, LAYUP_EINVAL, "round needs more than %d persistent launches", ctx->n_ps_ticket);
+        up.ps_ticket = ctx->d_ps_ticket + n_launch;
         const int grid = (int)std::min<long long>(tab.prefix[n], (long long)ctx->n_sm * ctx->ps_ctas);
         CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->ps_stages, ctx->ps_groups, ctx->ps_gs, ctx->pdl && n_launch == 0, s));
       } else {

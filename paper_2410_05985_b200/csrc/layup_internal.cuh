@@ -50,6 +50,8 @@ struct SchedParams {
   double *bpow;             // [L*K*2] (beta1^t, beta2^t) per (layer, replica), AdamW only
   double lr, beta1, beta2;  // fp32 values widened
   int32_t *ticket;          // [L] zero between launches; fused single-launch path only (update_tma.cu)
+  int32_t *ps_ticket;       // [n_ps_ticket] tile tickets of the persistent update launches behind this schedule
+  int32_t n_ps_ticket;      //   kernel (update_persist.cu); zeroed here
 };
 constexpr int kFusedMaxK = 64;         // the in-kernel schedule stage is O(K) per thread
 
@@ -69,6 +71,7 @@ struct UpdateParams {
   SchedParams sched;                // fused single-launch path: the schedule stage's inputs
   const void *tmaps;                // [n_sections][L] CUtensorMap (128 B each) of the layer sections, or nullptr
   unsigned long long *trace;        // [L] first CTA start per layer (%globaltimer, atomicMin), or nullptr (layup_trace)
+  int32_t *ps_ticket;               // persistent shape: this launch's tile ticket (zero at launch)
 };
 
 // layup_trace: the first CTA of a (step, layer) event to start leaves the GPU nanosecond timer

@@ -31,6 +31,8 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
   const int layer = p.layer_begin + blockIdx.x;
   const int i = threadIdx.x;
   const size_t row = (size_t)layer * K;
+  if (blockIdx.x == 0)                                           // tile tickets of the persistent update launches
+    for (int t = i; t < p.n_ps_ticket; t += blockDim.x) p.ps_ticket[t] = 0;
   // the round number is device state (layup.h "CUDA-graph capture"): every thread reads it here,
   // thread 0 advances it after the barrier below
   const uint32_t step = p.step_dev[layer];

@@ -13,8 +13,11 @@
 // Because G divides S a stage is always consumed by the same group, so every waiter of an mbarrier
 // sees each of its phases (a group that skipped a phase would mistake an older completion of the
 // same parity for its own).
-//   producers walk the CTA's share of the list (tile = blockIdx.x + n*gridDim.x, so the list is
-//             drained in order, output layer first); for each tile it waits for the stage's
+//   producers draw the CTA's next tile from a global ticket (one atomicAdd per tile by producer warp
+//             0, passed to the other warps through the stage), so the list is drained in order,
+//             output layer first, and an SM that runs slower simply takes fewer tiles (with a static
+//             stride a quarter of the SMs finished 2.7 ms after the rest on configs[2]);
+//             for each tile it waits for the stage's
 //             "empty" mbarrier, copies the layer's schedule tables (held in its registers, reloaded
 //             only when the list crosses into another layer) into the stage, and issues the tile's
 //             TMA loads on the stage's "full" mbarrier: ONE 2-D tiled load per array when every
@@ -81,7 +84,9 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
   // producers right after the local step, only the x slot (it holds y) lives through the mix
   uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)S * stage_f4);    // [S][NARR]
   uint64_t *empty = full + S * NARR;                                         // [S][NARR]
-  unsigned char *tables0 = reinterpret_cast<unsigned char *>(empty + S * NARR);   // [S] StageTables
+  uint64_t *sched = empty + S * NARR;                                        // [S] "tile number of the stage is known"
+  long long *tile_of = reinterpret_cast<long long *>(sched + S);             // [S] tile in the stage, -1 = list drained
+  unsigned char *tables0 = reinterpret_cast<unsigned char *>(tile_of + S);   // [S] StageTables
   const size_t tb = tables_bytes(K);
 
   if (threadIdx.x == 0) {
@@ -89,6 +94,7 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
       mbar_init(full + s, 1);
       mbar_init(empty + s, gthreads / 32);                // a stage is consumed by one group
     }
+    for (int s = 0; s < S; ++s) mbar_init(sched + s, 1);
   }
   __syncthreads();   // the only CTA-wide barrier: mbarriers visible
 
@@ -108,11 +114,39 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
     int pos = 0, cur_pos = -1, s = 0;
     uint32_t ph = 0;
     const float *const asrc = a == 0 ? p.x : a == 1 ? p.g : a == 2 ? p.m : p.v;
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    // the schedule kernel in front of this launch wrote the tables and zeroed the ticket
+    // (programmatic dependent launch: this kernel may have started under it)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    int sentinels = 0;
+    for (;;) {
+      // ---- which tile goes into stage s: warp 0 draws the ticket once its x slot is free
+      long long tile;
+      if (pw == 0) {
+        mbar_wait(empty + s * NARR, ph ^ 1u);             // the first trip round the ring is free
+        long long t = 0;
+        if (lane == 0) {
+          t = sentinels == 0 ? (long long)(unsigned)atomicAdd(p.ps_ticket, 1) : n_tiles;
+          if (t >= n_tiles) t = -1;
+          tile_of[s] = t;
+          ps_arrive(sched + s);                            // release: the other producer warps may read it
+        }
+        tile = __shfl_sync(0xFFFFFFFFu, t, 0);
+      } else {
+        mbar_wait(sched + s, ph);
+        tile = tile_of[s];
+        if (tile < 0) return;                             // list drained
+        mbar_wait(empty + s * NARR + a, ph ^ 1u);
+      }
+      if (tile < 0) {
+        // one end marker per consumer group (consecutive iterations belong to different groups)
+        __syncwarp();
+        if (lane == 0) ps_arrive(full + s * NARR);
+        if (++sentinels == G) return;
+        if (++s == S) { s = 0; ph ^= 1u; }
+        continue;
+      }
       while (tile >= tab.prefix[pos + 1]) ++pos;
       if (pos != cur_pos) {
-        // the schedule kernel in front of this launch wrote the tables (programmatic dependent launch)
-        if (cur_pos < 0) asm volatile("griddepcontrol.wait;" ::: "memory");
         const int layer = tab.layer[pos];
         const size_t row = (size_t)layer * K;
 #pragma unroll
@@ -139,8 +173,6 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
       const long long cols_left = (pad >> 2) - col0;
       const uint32_t chunk = (uint32_t)(cols_left < C ? cols_left : C) * 16u;
       uint64_t *const fbar = full + s * NARR + a;
-
-      mbar_wait(empty + s * NARR + a, ph ^ 1u);           // the first trip round the ring is free
       if (pw == 0) {
         // hand the layer's tables to the consumers through the stage (they acquire them with the x slot)
         const StageTables T = carve_tables(tables0 + (size_t)s * tb, K);
@@ -187,17 +219,18 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
       }
       if (++s == S) { s = 0; ph ^= 1u; }
     }
-    return;
   }
 
   // -------------------------------------------------------------------- consumer groups
   const int NT = gthreads;
   const int group = (int)threadIdx.x / gthreads, tid = (int)threadIdx.x % gthreads;
   int pos = 0, cur_pos = -1;
-  long long it = group;                                 // this group's iterations: group, group + G, ...
-  for (long long tile = blockIdx.x + it * gridDim.x; tile < n_tiles; tile += (long long)G * gridDim.x, it += G) {
-    const int s = (int)(it % S);
-    const uint32_t ph = (uint32_t)(it / S) & 1u;
+  int s = group;                                        // this group's iterations: group, group + G, ... (G divides S)
+  uint32_t ph = 0;
+  for (;;) {
+    mbar_wait(full + s * NARR, ph);                       // x slot, tables and the tile number have landed (acquire)
+    const long long tile = tile_of[s];
+    if (tile < 0) break;                                  // list drained
     while (tile >= tab.prefix[pos + 1]) ++pos;
     if (pos != cur_pos) {
       if (p.trace != nullptr && tid == 0) {             // layup_trace: first start of the layer on this GPU
@@ -219,7 +252,7 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
     float4 *ms = HAS_M ? gs + n_items : gs, *vs = HAS_V ? ms + n_items : ms;
     const StageTables T = carve_tables(tables0 + (size_t)s * tb, K);
 #pragma unroll
-    for (int a = 0; a < NARR; ++a) mbar_wait(full + s * NARR + a, ph);   // tile and tables have landed (acquire)
+    for (int a = 1; a < NARR; ++a) mbar_wait(full + s * NARR + a, ph);   // the other arrays of the tile
 
     // ---- phase 1: local step; y overwrites x in place, m' (v') -> HBM
     for (int idx = tid; idx < n_items; idx += NT) {
@@ -265,6 +298,8 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
     fence_proxy_async();   // the x slot was written through the generic proxy; the TMA engine refills it next
     __syncwarp();
     if ((tid & 31) == 0) ps_arrive(empty + s * NARR);     // this warp is done with the stage
+    s += G;
+    if (s >= S) { s -= S; ph ^= 1u; }
   }
 }
 
@@ -275,7 +310,7 @@ const PsFn kPs[3][2] = {{layup_update_persist<OPT_SGD, false>, layup_update_pers
 
 size_t stage_bytes(int K, int C, int opt) {
   const int narr = opt == OPT_ADAMW ? 4 : opt == OPT_SGD_MOM ? 3 : 2;
-  return (size_t)K * C * sizeof(float4) * narr + 16 * (size_t)narr + tables_bytes(K);   // arrays, mbarrier pairs, tables
+  return (size_t)K * C * sizeof(float4) * narr + 16 * (size_t)narr + 16 + tables_bytes(K);   // arrays, mbarrier pairs, tile number + its barrier, tables
 }
 
 }  // namespace
