@@ -81,13 +81,20 @@ typedef struct {
                            schedule stage inside the update kernel (ONE launch); 2: never            */
   int32_t fused_waves;  /* default 4                                                                */
   int32_t tile_items;   /* float4 items (replicas x columns) per work item; default 1024            */
-  int32_t variant;      /* grouped shape: thread shape of the update kernel (index; 0 = default);
+  int32_t variant;      /* grouped shape: thread shape of the update kernel, an index into update_tma.cu's
+                           table (0 = the library's choice; 1 128 threads x 8 CTAs/SM, 2 512 x 2,
+                           3 256 x 2, 4 512 x 3, 5 256 x 5 with the last array of x, g, m, v staged
+                           through registers instead of shared memory -- what straggler-mode launches
+                           take by default when the optimiser has state);
                            persistent shape: consumer groups per CTA (0 = as many as the ring feeds) */
   int32_t ctas_per_sm;  /* cap on resident CTAs per SM of persistent grids; default: all that fit   */
   int32_t pdl;          /* 0 auto = 1; 1: the update kernel is a programmatic dependent launch behind
                            the schedule kernel; 2: plain stream order                               */
-  int32_t tma2d;        /* 0 auto (by K and optimiser); 1: one 2-D tiled TMA load per
-                           array and tile; 2: K 1-D bulk copies per array and tile                  */
+  int32_t tma2d;        /* 0 auto (by K and optimiser); 1: tensor-map loads -- one 2-D tiled
+                           TMA load per array and tile, and in straggler mode (skip_prob > 0 or a delay
+                           straggler) tile::gather4 requests of four replica rows each; 2: 1-D bulk
+                           copies, one per (replica, array) row the round needs (the straggler-mode
+                           default)                                                                  */
   int32_t stages;       /* persistent shape: depth of the TMA ring; default: as deep as fits        */
   int32_t group_threads;/* persistent shape: threads per consumer group (multiple of 32); default
                            512 with one group, 256 with more                                        */

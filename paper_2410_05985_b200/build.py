@@ -8,7 +8,7 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(CSRC, "liblayup.so")
 SOURCES = ["api.cu", "schedule.cu", "update.cu", "update_tma.cu", "update_persist.cu", "diagnose.cu"]
 HEADERS = ["layup_internal.cuh", "philox.cuh", "rule.cuh", "tma_ptx.cuh", os.path.join("..", "..", "include", "layup.h")]
-NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+NVCC_FLAGS = ["-O3", "-std=c++17", "--threads", "0", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
 
 

@@ -33,6 +33,9 @@ struct layup_ctx {
   int C = 0, log2C = 0, smem = 0, ctas_per_sm = 1, n_sm = 1;
   layup_tuning tune{};                                 // layup_config.tuning (zeros = defaults)
   int variant = 0, threads = 256;
+  int rega = 0;                                        // arrays the thread shape stages through registers
+  bool straggler_mode = false;                         // skip_prob > 0 or a delay-mode straggler
+  int split_variant = -1, split_smem = 0;              // straggler mode: thread shape of the non-fused launches (-1: ctx->variant)
   bool persistent = false;                             // tuning.launch_shape == 2
   int engine = 1;                                      // 1: TMA-staged kernel, 0: LDG kernel
   int32_t delay_replica = 0, delay_rounds = 0;
@@ -46,6 +49,7 @@ struct layup_ctx {
   SchedTables t{};
   int32_t *d_peer_scratch = nullptr, *d_ticket = nullptr;
   void *d_tmaps = nullptr;                // [n_sections][L] CUtensorMap: 2-D tiled view [K][pad] of every layer section
+  void *d_tmaps_g4 = nullptr;             // ... with a one-row box, for tile::gather4 (straggler mode, grouped shape)
   bool ps_ok = false;                     // tuning.launch_shape == 2: persistent form of the TMA kernel
   int ps_smem = 0, ps_ctas = 0, ps_stages = 0, ps_groups = 1, ps_gs = 256;
   bool pdl = true;                        // programmatic dependent launch of the update kernel behind the schedule kernel
@@ -258,6 +262,11 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     return bail(LAYUP_EINVAL);
   }
   ctx->engine = tune.engine == 2 ? 0 : 1;
+  ctx->straggler_mode = ctx->skip_thr != 0u || ctx->delay_rounds != 0;     // some replicas may idle in a round
+  // Straggler mode fetches exactly the rows a round needs.  tma2d = 1 asks for tile::gather4 requests
+  // (four rows each); measured on B200 it does not beat row-by-row bulk copies, which
+  // stay the default.
+  const bool want_g4 = ctx->straggler_mode && tune.launch_shape != 2 && tune.tma2d == 1 && C * 4 <= 256;
   ctx->persistent = tune.launch_shape == 2;
   ctx->variant = (ctx->persistent && tune.engine != 2) ? 0 : tune.variant;   // persistent TMA shape: variant = consumer groups
   ctx->pdl = tune.pdl != 2;
@@ -266,12 +275,28 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
     if (ctx->variant < 0 || ctx->variant >= tma_num_variants()) ctx->variant = 0;
     if (tune.variant == 0) ctx->variant = tma_default_variant(K * C, ctx->n_sections);
     ctx->fused_ok = K <= kFusedMaxK && tma_has_fused(ctx->variant) && tune.fused != 2;
-    const size_t need_smem = tma_smem_bytes(K, C, ctx->opt, ctx->fused_ok);
+    ctx->rega = tma_variant_rega(ctx->variant, ctx->opt);
+    const int max_items = tma_variant_max_items(ctx->variant);
+    if (max_items > 0 && K * C > max_items) {
+      fail(nullptr, LAYUP_EINVAL, "thread shape %d takes tiles of at most %d items (this ctx: %d)", ctx->variant, max_items, K * C);
+      return bail(LAYUP_EINVAL);
+    }
+    const size_t need_smem = tma_smem_bytes(K, C, ctx->opt, ctx->fused_ok, ctx->rega, want_g4);
     if (need_smem > prop.sharedMemPerBlockOptin) { ctx->engine = 0; ctx->fused_ok = false; }
     else ctx->smem = (int)need_smem;
   }
   if (ctx->engine == 1) {
-    CU_TRY_INIT(tma_kernel_setup(ctx->variant, ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
+    CU_TRY_INIT(tma_kernel_setup(ctx->variant, ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->straggler_mode, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
+    // Straggler mode with optimiser state: launches that are not latency bound take the split-staged
+    // shape (last array through registers, five CTAs per SM)
+    if (tune.variant == 0 && ctx->straggler_mode) {
+      ctx->split_variant = tma_split_variant(K * C, ctx->n_sections);
+      if (ctx->split_variant >= 0) {
+        int thr = 0, occ = 0;
+        ctx->split_smem = (int)tma_smem_bytes(K, C, ctx->opt, false, tma_variant_rega(ctx->split_variant, ctx->opt), want_g4);
+        CU_TRY_INIT(tma_kernel_setup(ctx->split_variant, ctx->opt, ctx->mix_mode == kMixSymmetric, true, ctx->split_smem, &thr, &occ));
+      }
+    }
   } else {
     if (ctx->variant < 0 || ctx->variant >= update_num_variants()) ctx->variant = 0;
     CU_TRY_INIT(update_kernel_setup(ctx->variant, ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
@@ -322,10 +347,14 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   // clear win without momentum (K = 16: 6.27 -> 6.94 TB/s) and from 64 copies per CTA up; at
   // K = 16 with momentum (48 copies) the 1-D form is 0.2 % ahead, so it is kept there.
   // (the persistent shape issues a tile's loads from one warp: always the 2-D form there)
-  const bool want_2d = tune.tma2d == 1 || (tune.tma2d == 0 && (ctx->n_sections == 2 || K * ctx->n_sections >= 64 || ctx->persistent));
-  if (ctx->engine == 1 && want_2d && K <= 256 && C * 4 <= 256) {
+  // Straggler mode with tma2d = 1 (grouped shape): the same views with a ONE-row box, read four
+  // arbitrary rows at a time with tile::gather4.
+  const int n_staged = ctx->n_sections - ctx->rega;
+  const bool want_2d = tune.tma2d == 1 || (tune.tma2d == 0 && (n_staged <= 2 || K * n_staged >= 64 || ctx->persistent));
+  if (ctx->engine == 1 && C * 4 <= 256 && (want_g4 || (!ctx->straggler_mode && want_2d && K <= 256))) {
     // One tensor map per (section, layer): rank 2, inner dim = the padded slice, outer dim = the K
-    // replicas (stride = pad), box = [K][C*4 floats], no swizzle, zero fill past the slice end.
+    // replicas (stride = pad), box = [K][C*4 floats] ([1][C*4] for gather4), no swizzle, zero fill
+    // past the slice end.
     typedef CUresult (*EncodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -340,7 +369,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
         if (d.pad >= (1ll << 31)) { ok = false; break; }                  // box coordinates are int32
         const cuuint64_t gdim[2] = {(cuuint64_t)d.pad, (cuuint64_t)K};
         const cuuint64_t gstride[1] = {(cuuint64_t)d.pad * sizeof(float)};
-        const cuuint32_t box[2] = {(cuuint32_t)(C * 4), (cuuint32_t)K};
+        const cuuint32_t box[2] = {(cuuint32_t)(C * 4), want_g4 ? 1u : (cuuint32_t)K};
         const cuuint32_t estride[2] = {1, 1};
         void *base_ptr = ctx->arena + (long long)a * ctx->section + d.base;
         ok = ((EncodeTiled)fn)(&maps[(size_t)a * L + l], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base_ptr, gdim, gstride, box,
@@ -349,8 +378,9 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
       }
     cudaGetLastError();
     if (ok) {
-      CU_TRY_INIT(cudaMalloc(&ctx->d_tmaps, sizeof(CUtensorMap) * maps.size()));
-      CU_TRY_INIT(cudaMemcpy(ctx->d_tmaps, maps.data(), sizeof(CUtensorMap) * maps.size(), cudaMemcpyHostToDevice));
+      void **slot = want_g4 ? &ctx->d_tmaps_g4 : &ctx->d_tmaps;
+      CU_TRY_INIT(cudaMalloc(slot, sizeof(CUtensorMap) * maps.size()));
+      CU_TRY_INIT(cudaMemcpy(*slot, maps.data(), sizeof(CUtensorMap) * maps.size(), cudaMemcpyHostToDevice));
     }
   }
   if (ctx->engine == 1 && ctx->persistent) {
@@ -412,7 +442,7 @@ extern "C" int layup_destroy(layup_ctx *ctx) {
   cudaFree(ctx->d_layers); cudaFree(ctx->d_tile_prefix); cudaFree(ctx->d_w);
   cudaFree(ctx->t.peer); cudaFree(ctx->t.recv_off); cudaFree(ctx->t.senders); cudaFree(ctx->t.alpha);
   cudaFree(ctx->t.c1); cudaFree(ctx->t.c2); cudaFree(ctx->d_bpow);
-  cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_ticket); cudaFree(ctx->d_tmaps);
+  cudaFree(ctx->t.flags); cudaFree(ctx->d_peer_scratch); cudaFree(ctx->d_ticket); cudaFree(ctx->d_tmaps); cudaFree(ctx->d_tmaps_g4);
   cudaFree(ctx->d_active_scratch); cudaFree(ctx->d_dist); cudaFree(ctx->d_step); cudaFree(ctx->d_trace); cudaFree(ctx->d_ps_ticket);
   delete ctx;
   return LAYUP_OK;
@@ -475,6 +505,7 @@ static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_
   up.all_active = (ctx->skip_thr == 0u && ctx->delay_rounds == 0) ? 1 : 0;
   up.sched = sp;
   up.tmaps = ctx->d_tmaps;
+  up.tmaps_g4 = ctx->d_tmaps_g4;
   up.trace = ctx->tracing ? ctx->d_trace : nullptr;
   const long long tiles = up.tile_end - up.tile_begin;
   const long long resident = (long long)ctx->n_sm * ctx->ctas_per_sm;
@@ -502,7 +533,9 @@ static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_
         const int grid = (int)std::min<long long>(tab.prefix[n], (long long)ctx->n_sm * ctx->ps_ctas);
         CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->ps_stages, ctx->ps_groups, ctx->ps_gs, ctx->pdl && n_launch == 0, s));
       } else {
-        CU_TRY(ctx, launch_update_tma(up, tab, ctx->variant, fused, ctx->pdl && n_launch == 0, (int)tab.prefix[n], ctx->smem, s));
+        const bool split = !fused && ctx->split_variant >= 0;
+        CU_TRY(ctx, launch_update_tma(up, tab, split ? ctx->split_variant : ctx->variant, fused, ctx->pdl && n_launch == 0,
+                                      (int)tab.prefix[n], split ? ctx->split_smem : ctx->smem, s));
       }
       q0 += n;
       ++n_launch;

@@ -70,6 +70,7 @@ struct UpdateParams {
   int32_t all_active;               // skip_prob == 0: every replica is active in every round
   SchedParams sched;                // fused single-launch path: the schedule stage's inputs
   const void *tmaps;                // [n_sections][L] CUtensorMap (128 B each) of the layer sections, or nullptr
+  const void *tmaps_g4;             // same views with a one-row box, for tile::gather4 (straggler mode), or nullptr
   unsigned long long *trace;        // [L] first CTA start per layer (%globaltimer, atomicMin), or nullptr (layup_trace)
   int32_t *ps_ticket;               // persistent shape: this launch's tile ticket (zero at launch)
 };
@@ -112,9 +113,12 @@ size_t update_smem_bytes(int K, int C);
 // update_tma.cu -- TMA-bulk staged variants
 int tma_num_variants();
 int tma_default_variant(int n_items, int n_sections);
-size_t tma_smem_bytes(int K, int C, int opt, bool fused);
+int tma_split_variant(int n_items, int n_sections);
+size_t tma_smem_bytes(int K, int C, int opt, bool fused, int rega, bool gather4);
+int tma_variant_rega(int variant, int opt);        // arrays this thread shape stages through registers
+int tma_variant_max_items(int variant);            // ... and the largest tile it takes (0 = any)
 bool tma_has_fused(int variant);
-cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_bytes, int *threads, int *ctas_per_sm);
+cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, bool strag, int smem_bytes, int *threads, int *ctas_per_sm);
 cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, bool pdl, int grid,
                               int smem_bytes, cudaStream_t s);
 

@@ -6,14 +6,23 @@
 //   - when every replica is active and the box fits the TMA limits: ONE 2-D tiled copy per array
 //     (cp.async.bulk.tensor.2d, SASS UTMALDG.2D) through a tensor map that views a layer section
 //     as [K rows][padded slice];
-//   - otherwise K x arrays 1-D bulk copies (cp.async.bulk, SASS UBLKCP), spread over all warps,
-//     skipping what an idle replica does not need.
+//   - all active but no tensor map (K > 256, huge slices): K x arrays 1-D bulk copies (cp.async.bulk,
+//     SASS UBLKCP), spread over all warps;
+//   - straggler mode (STRAG): the rows a round needs -- x of every replica that is active or
+//     receives, g / m / v of the active ones -- are only known on the device.  They are fetched in
+//     groups of four consecutive replicas with cp.async.bulk.tensor.2d.tile::gather4 (SASS
+//     UTMALDG.2D.GATHER4: four arbitrary rows of the [K][padded slice] view per request; a row the
+//     round does not need is given an out-of-range index, which costs no HBM traffic and lands as
+//     zeros), so an idle replica costs no bytes and a tile issues a quarter of the requests that
+//     row-by-row copies need.
 // The local step then runs out of shared memory, y overwrites x in place (the "send" is an
 // on-chip read), m' (and AdamW's v') go straight to HBM, and after one CTA barrier
 // every receiver folds its senders and writes x once.  HBM traffic: 12 B (SGD) / 20 B (momentum) /
 // 28 B (AdamW) per parameter update, nothing read or written twice.
 // Template parameters: OPT = local optimiser (rule.cuh), SYM = symmetric pairwise averaging
-// instead of the push-sum fold, FUSED = the schedule stage runs in this kernel (one launch).
+// instead of the push-sum fold, FUSED = the schedule stage runs in this kernel (one launch),
+// STRAG = the ctx has a straggler mode (some replicas may idle: compacted rows),
+// REGA / U = split staging (below).
 #include "layup_internal.cuh"
 #include "philox.cuh"
 #include "rule.cuh"
@@ -28,19 +37,37 @@ namespace {
 // shared memory from the same inputs (seed, step, w, beta powers), so all CTAs agree bit for bit;
 // the CTA that is LAST to have read the state (a ticket per layer) writes the new w / beta powers
 // back in place.  Used for launches of few tiles (launch-latency bound) and K <= kFusedMaxK.
-template <int OPT, bool SYM, bool FUSED, int THREADS, int MINB>
+__device__ __forceinline__ float4 ld4_stream(const float *p) {   // read once, by this thread only: keep it out of L1
+  float4 v;
+  asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
+  return v;
+}
+
+// REGA / U: split staging.  Only x has to be in shared memory (it becomes y, which the receivers
+// of other replicas read); g, m and v are consumed once, by the thread that takes the local step
+// of that element.  REGA > 0 brings the LAST REGA arrays of (x, g, m, v) into REGISTERS with plain
+// 128-bit loads issued next to the TMA copies (each thread owns U items: idx = tid + u*THREADS),
+// so a CTA needs less shared memory and one more CTA fits per SM (straggler rounds).
+template <int OPT, bool SYM, bool FUSED, bool STRAG, int THREADS, int MINB, int REGA = 0, int U = 1>
 __global__ void __launch_bounds__(THREADS, MINB)
     layup_update_tma(const __grid_constant__ UpdateParams p, const __grid_constant__ PosTable tab) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int NARR = OptTraits<OPT>::kArrays;
   constexpr bool HAS_M = NARR >= 3, HAS_V = NARR >= 4;
+  constexpr int RA = REGA < NARR ? REGA : NARR - 1;                         // arrays staged through registers
+  constexpr int NS = NARR - RA;                                             // arrays staged in shared memory
+  constexpr bool G_REG = NS <= 1, M_REG = HAS_M && NS <= 2, V_REG = HAS_V && NS <= 3;
+  constexpr int NW = THREADS / 32;
+  static_assert(!(FUSED && RA > 0), "the single-launch path stages every array in shared memory");
   const int K = p.K, C = p.C, log2C = p.log2C, tid = threadIdx.x;
   const int n_items = K << log2C;
+  const int arr_items = STRAG && p.tmaps_g4 != nullptr ? ((K + 3) & ~3) << log2C : n_items;   // gather4: whole groups of four rows
   float4 *xs = reinterpret_cast<float4 *>(smem_raw);                       // [K*C]  x, then y in place
-  float4 *gs = xs + n_items;                                                // [K*C]
-  float4 *ms = HAS_M ? gs + n_items : gs;                                   // [K*C] (momentum / Adam m)
-  float4 *vs = HAS_V ? ms + n_items : ms;                                   // [K*C] (Adam v)
-  uint64_t *bar = reinterpret_cast<uint64_t *>(xs + NARR * n_items);
+  float4 *gs = xs + arr_items;                                              // [K*C]  (unless G_REG)
+  float4 *ms = HAS_M ? gs + arr_items : gs;                                 // [K*C] (momentum / Adam m; unless M_REG)
+  float4 *vs = HAS_V ? ms + arr_items : ms;                                 // [K*C] (Adam v; unless V_REG)
+  uint64_t *bar = reinterpret_cast<uint64_t *>(xs + NS * arr_items);
   double *s_wh = reinterpret_cast<double *>(bar + 1);                       // [K]  FUSED only: halved weights
   double *s_wnew = s_wh + (FUSED ? K : 0);                                  // [K]  FUSED only: w after the round
   double *s_bp = s_wnew + (FUSED ? K : 0);                                  // [2K] FUSED + AdamW: new beta powers
@@ -51,7 +78,7 @@ __global__ void __launch_bounds__(THREADS, MINB)
   float *s_alpha = reinterpret_cast<float *>(s_peer + (FUSED ? K : 0));     // [K]
   float *s_c1 = s_alpha + K;                                                // [K]  (AdamW only)
   float *s_c2 = s_c1 + (HAS_V ? K : 0);                                     // [K]  (AdamW only)
-  unsigned char *s_flags = reinterpret_cast<unsigned char *>(s_c2 + (HAS_V ? K : 0));  // [K]
+  unsigned char *s_flags = reinterpret_cast<unsigned char *>(s_c2 + (HAS_V ? K : 0));  // [K rounded up to 4], 4-byte aligned
 
   if (FUSED) {
     // Launched as a programmatic dependent of whatever kernel precedes it on the stream (in a graph
@@ -82,40 +109,72 @@ __global__ void __launch_bounds__(THREADS, MINB)
   const uint32_t chunk = (uint32_t)ncols * 16u;
 
   trace_start(p.trace, layer);
-  const bool boxed = p.all_active && p.tmaps != nullptr;   // whole-tile 2-D TMA loads, one per array
+  const bool boxed = !STRAG && p.tmaps != nullptr;         // whole-tile 2-D TMA loads, one per array
   if (tid == 0) {
-    mbar_init(bar, 1);
-    // no straggler this round: every replica is active, the byte count is known up front
+    // STRAG: every warp posts the bytes of the copies it issues and then arrives (NW arrivals);
+    // otherwise every replica is active, the byte count is known up front and thread 0 alone arrives
+    mbar_init(bar, STRAG ? NW : 1);
+    if (STRAG)
+      for (int k = K; k < ((K + 3) & ~3); ++k) s_flags[k] = 0;              // the last group of four may be partial
     if (boxed) {
-      mbar_expect_tx(bar, (uint32_t)n_items * 16u * NARR);                  // full boxes, zero fill included
+      mbar_expect_tx(bar, (uint32_t)n_items * 16u * NS);                    // full boxes, zero fill included
       const unsigned char *tm = reinterpret_cast<const unsigned char *>(p.tmaps);
 #pragma unroll
-      for (int a = 0; a < NARR; ++a)
-        tma_load_2d(xs + a * n_items, tm + ((size_t)a * p.L + layer) * 128, (int)(col0 << 2), 0, bar);
-    } else if (p.all_active) {
-      mbar_expect_tx(bar, (uint32_t)K * NARR * chunk);
+      for (int a = 0; a < NS; ++a)
+        tma_load_2d(xs + a * arr_items, tm + ((size_t)a * p.L + layer) * 128, (int)(col0 << 2), 0, bar);
+    } else if (!STRAG) {
+      mbar_expect_tx(bar, (uint32_t)K * NS * chunk);
     }
   }
   __syncthreads();   // mbarrier visible
 
   // Bulk copies are issued one lane at a time within a warp, so spread them over all warps:
-  // copy slot c = (replica, array) goes to warp c % NW, lane c / NW.
-  constexpr int NW = THREADS / 32;
+  // copy slot c goes to warp c % NW, lane c / NW.
   const int slot0 = (tid & 31) * NW + (tid >> 5);
-  auto issue_copies = [&](bool use_flags) {
-    for (int c = slot0; c < K * NARR; c += THREADS) {
-      const int i = c / NARR, a = c - i * NARR;
-      if (use_flags) {
-        const int f = s_flags[i];
-        if (!f || (a > 0 && !(f & kFlagActive))) continue;
+  if (!STRAG && !boxed) {
+    for (int c = slot0; c < K * NS; c += THREADS) {
+      const int i = c / NS, a = c - i * NS;
+      const float *src = (a == 0 ? xb : a == 1 ? gb : a == 2 ? mb : vb) + (long long)i * pad;
+      bulk_g2s(xs + a * arr_items + (i << log2C), src, chunk, bar);
+    }
+  }
+
+  // Straggler mode, row copies: slot c = (replica i, array a) is fetched iff the round needs it -- x
+  // of a replica that is active or receives, g / m / v of an active one (an idle replica costs no
+  // bytes).  Every thread posts the bytes of its own copies on the barrier, and every warp arrives
+  // once its lanes have posted, so the phase cannot complete before the last byte count is known.
+  bool rows_issued = false;
+  auto issue_rows = [&](auto flag_of) {
+    for (int c = slot0; c < K * NS; c += THREADS) {
+      const int i = c / NS, a = c - i * NS;
+      const int f = flag_of(i);
+      if (!f || (a > 0 && !(f & kFlagActive))) continue;
+      const float *src = (a == 0 ? xb : a == 1 ? gb : a == 2 ? mb : vb) + (long long)i * pad;
+      mbar_post_tx(bar, chunk);
+      bulk_g2s(xs + a * arr_items + (i << log2C), src, chunk, bar);
+    }
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(bar);
+  };
+
+  // register-staged arrays: this thread's U items, requested while the TMA copies are in flight
+  const float4 zero4 = float4{0.f, 0.f, 0.f, 0.f};
+  float4 rg[RA > 0 ? U : 1], rm[RA > 0 ? U : 1], rv[RA > 0 ? U : 1];
+  auto reg_loads = [&]() {
+#pragma unroll
+    for (int u = 0; u < (RA > 0 ? U : 0); ++u) {
+      const int idx = tid + u * THREADS;
+      const int i = idx >> log2C, c = idx & (C - 1);
+      rg[u] = rm[u] = rv[u] = zero4;
+      if (idx < n_items && c < ncols && (!STRAG || (s_flags[i] & kFlagActive))) {
+        const long long off = (long long)i * pad + (c << 2);
+        if (G_REG) rg[u] = ld4_stream(gb + off);
+        if (M_REG) rm[u] = ld4_stream(mb + off);
+        if (V_REG) rv[u] = ld4_stream(vb + off);
       }
-      const long long off = (long long)i * pad;
-      void *dst = xs + a * n_items + (i << log2C);
-      const float *src = (a == 0 ? xb : a == 1 ? gb : a == 2 ? mb : vb) + off;
-      bulk_g2s(dst, src, chunk, bar);
     }
   };
-  if (p.all_active && !boxed) issue_copies(false);
+  if (RA > 0 && !STRAG) reg_loads();
 
   // this layer's schedule -> shared memory (overlaps the bulk copies when all replicas are active)
   int ticket = -1;
@@ -202,6 +261,12 @@ __global__ void __launch_bounds__(THREADS, MINB)
     // on the stream is still running (its tile loads above do not depend on it); the tables do.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     const size_t row = (size_t)layer * K;
+    if (STRAG && p.tmaps_g4 == nullptr) {
+      // every copy depends on ONE flag only: read it straight from the device table and issue, without
+      // waiting for the tables to be staged in shared memory
+      issue_rows([&](int i) { return (int)p.t.flags[row + i]; });
+      rows_issued = true;
+    }
     for (int k = tid; k < K; k += THREADS) {
       s_senders[k] = SYM ? p.t.peer[row + k] : p.t.senders[row + k];
       s_alpha[k] = p.t.alpha[row + k];
@@ -217,35 +282,58 @@ __global__ void __launch_bounds__(THREADS, MINB)
     __syncthreads();   // schedule visible
   }
 
-  if (!p.all_active) {
-    // straggler round: the flags decide which chunks are touched at all
-    if (tid < 32) {
-      uint32_t bytes = 0;
-      for (int i = tid; i < K; i += 32) {
-        const int f = s_flags[i];
-        bytes += f ? chunk * ((f & kFlagActive) ? (uint32_t)NARR : 1u) : 0u;
-      }
+  if (STRAG) {
+    if (p.tmaps_g4 != nullptr) {
+      // tile::gather4: request slot c = (group q of four consecutive replicas, array a); a row the
+      // round does not need gets the row index K, which does not exist: no HBM traffic, zeros in
+      // shared memory (never read)
+      const int n_groups = (K + 3) >> 2;
+      const unsigned char *tm = reinterpret_cast<const unsigned char *>(p.tmaps_g4);
+      for (int c = slot0; c < n_groups * NS; c += THREADS) {
+        const int q = c / NS, a = c - q * NS;
+        const uint32_t f4 = *reinterpret_cast<const uint32_t *>(s_flags + 4 * q);     // flags of replicas 4q .. 4q+3
+        const uint32_t need = a == 0 ? (f4 | (f4 >> 1)) & 0x01010101u : f4 & 0x01010101u;   // kFlagActive = 1, kFlagRecv = 2
+        if (need == 0u) continue;
+        int r4[4];
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xFFFFFFFFu, bytes, o);
-      if (tid == 0) mbar_expect_tx(bar, bytes);
+        for (int j = 0; j < 4; ++j) r4[j] = (need >> (8 * j)) & 1u ? 4 * q + j : K;
+        mbar_post_tx(bar, 4u * (uint32_t)C * 16u);
+        tma_gather4(xs + a * arr_items + ((4 * q) << log2C), tm + ((size_t)a * p.L + layer) * 128, (int)(col0 << 2),
+                    r4[0], r4[1], r4[2], r4[3], bar);
+      }
+      __syncwarp();
+      if ((tid & 31) == 0) mbar_arrive(bar);
+    } else if (!rows_issued) {
+      issue_rows([&](int i) { return (int)s_flags[i]; });
     }
-    __syncthreads();
-    issue_copies(true);
+    if (RA > 0) reg_loads();
   }
   mbar_wait(bar, 0);
 
   // ---- phase 1: local step out of shared memory; y overwrites x in place, m' (v') -> HBM
-  for (int idx = tid; idx < n_items; idx += THREADS) {
+  auto step_item = [&](int idx, const float4 &g, float4 m, float4 v) {
     const int i = idx >> log2C, c = idx & (C - 1);
-    if (c >= ncols) continue;
-    if (!(s_flags[i] & kFlagActive)) continue;                              // idle replica: y = x already there
-    float4 m = HAS_M ? ms[idx] : float4{0.f, 0.f, 0.f, 0.f};
-    float4 v = HAS_V ? vs[idx] : float4{0.f, 0.f, 0.f, 0.f};
-    const float4 y = local_step4<OPT>(xs[idx], gs[idx], m, v, p.s, HAS_V ? s_c1[i] : 0.f, HAS_V ? s_c2[i] : 0.f);
+    const float4 y = local_step4<OPT>(xs[idx], g, m, v, p.s, HAS_V ? s_c1[i] : 0.f, HAS_V ? s_c2[i] : 0.f);
     const long long off = (long long)i * pad + (c << 2);
     if (HAS_M) st4(mb + off, m);
     if (HAS_V) st4(vb + off, v);
     xs[idx] = y;
+  };
+  if (RA == 0) {
+    for (int idx = tid; idx < n_items; idx += THREADS) {
+      if ((idx & (C - 1)) >= ncols) continue;
+      if (STRAG && !(s_flags[idx >> log2C] & kFlagActive)) continue;        // idle replica: y = x already there
+      step_item(idx, gs[idx], HAS_M ? ms[idx] : zero4, HAS_V ? vs[idx] : zero4);
+    }
+  } else {
+#pragma unroll
+    for (int u = 0; u < (RA > 0 ? U : 0); ++u) {
+      const int idx = tid + u * THREADS;
+      if (idx >= n_items || (idx & (C - 1)) >= ncols) continue;
+      if (STRAG && !(s_flags[idx >> log2C] & kFlagActive)) continue;
+      step_item(idx, G_REG ? rg[u] : gs[idx], HAS_M ? (M_REG ? rm[u] : ms[idx]) : zero4,
+                HAS_V ? (V_REG ? rv[u] : vs[idx]) : zero4);
+    }
   }
   __syncthreads();
 
@@ -256,7 +344,7 @@ __global__ void __launch_bounds__(THREADS, MINB)
     __syncthreads();
     for (int idx = tid; idx < n_items; idx += THREADS) {
       const int i = idx >> log2C, c = idx & (C - 1);
-      if (c >= ncols || !s_flags[i]) continue;                              // idle and nobody's peer: 0 bytes
+      if (c >= ncols || (STRAG && !s_flags[i])) continue;                   // idle and nobody's peer: 0 bytes
       st4(xb + (long long)i * pad + (c << 2), xs[idx]);
     }
   } else {
@@ -264,7 +352,7 @@ __global__ void __launch_bounds__(THREADS, MINB)
     for (int idx = tid; idx < n_items; idx += THREADS) {
       const int i = idx >> log2C, c = idx & (C - 1);
       if (c >= ncols) continue;
-      if (!s_flags[i]) continue;                                            // idle, no push received: 0 bytes
+      if (STRAG && !s_flags[i]) continue;                                   // idle, no push received: 0 bytes
       float4 acc = xs[idx];
       const int k0 = s_begin[i], k_end = k0 + s_cnt[i];
       for (int k = k0; k < k_end; ++k) peer_update4(acc, xs[(s_senders[k] << log2C) + c], s_alpha[k]);
@@ -320,46 +408,67 @@ __global__ void __launch_bounds__(THREADS, MINB)
 using TmaFn = void (*)(const UpdateParams, const PosTable);
 struct TmaVariant {
   int threads, minb;
-  TmaFn fn[3][2];       // [OPT][SYM]   schedule tables read from global memory (two launches)
-  TmaFn fused[3][2];    // [OPT][SYM]   schedule computed in the kernel (one launch); nullptr = not built
+  int rega, items;      // split staging: arrays through registers, items per thread (0, 0 = everything in shared memory)
+  TmaFn fn[2][3][2];    // [STRAG][OPT][SYM]   schedule tables read from global memory (two launches)
+  TmaFn fused[2][3][2]; // [STRAG][OPT][SYM]   schedule computed in the kernel (one launch); nullptr = not built
 };
-#define LAYUP_TMA_ROW(O, F, T, MB) {layup_update_tma<O, false, F, T, MB>, layup_update_tma<O, true, F, T, MB>}
-#define LAYUP_TMA_TABLE(F, T, MB) \
-  {LAYUP_TMA_ROW(OPT_SGD, F, T, MB), LAYUP_TMA_ROW(OPT_SGD_MOM, F, T, MB), LAYUP_TMA_ROW(OPT_ADAMW, F, T, MB)}
-#define LAYUP_TMA_NONE {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}}
+#define LAYUP_TMA_ROW(O, F, ST, T, MB, R, UU) \
+  {layup_update_tma<O, false, F, ST, T, MB, R, UU>, layup_update_tma<O, true, F, ST, T, MB, R, UU>}
+#define LAYUP_TMA_OPTS(F, ST, T, MB, R, UU)                                                      \
+  {LAYUP_TMA_ROW(OPT_SGD, F, ST, T, MB, R, UU), LAYUP_TMA_ROW(OPT_SGD_MOM, F, ST, T, MB, R, UU), \
+   LAYUP_TMA_ROW(OPT_ADAMW, F, ST, T, MB, R, UU)}
+#define LAYUP_TMA_TABLE(F, T, MB, R, UU) {LAYUP_TMA_OPTS(F, false, T, MB, R, UU), LAYUP_TMA_OPTS(F, true, T, MB, R, UU)}
+#define LAYUP_TMA_NONE6 {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}}
+#define LAYUP_TMA_NONE {LAYUP_TMA_NONE6, LAYUP_TMA_NONE6}
 const TmaVariant kTma[] = {
-    TmaVariant{256, 4, LAYUP_TMA_TABLE(false, 256, 4), LAYUP_TMA_TABLE(true, 256, 4)},
-    TmaVariant{128, 8, LAYUP_TMA_TABLE(false, 128, 8), LAYUP_TMA_NONE},
-    TmaVariant{512, 2, LAYUP_TMA_TABLE(false, 512, 2), LAYUP_TMA_NONE},
-    TmaVariant{256, 2, LAYUP_TMA_TABLE(false, 256, 2), LAYUP_TMA_NONE},
+    TmaVariant{256, 4, 0, 0, LAYUP_TMA_TABLE(false, 256, 4, 0, 1), LAYUP_TMA_TABLE(true, 256, 4, 0, 1)},
+    TmaVariant{128, 8, 0, 0, LAYUP_TMA_TABLE(false, 128, 8, 0, 1), LAYUP_TMA_NONE},
+    TmaVariant{512, 2, 0, 0, LAYUP_TMA_TABLE(false, 512, 2, 0, 1), LAYUP_TMA_NONE},
+    TmaVariant{256, 2, 0, 0, LAYUP_TMA_TABLE(false, 256, 2, 0, 1), LAYUP_TMA_NONE},
     // tiles of >= 2048 items (K >= 32 without momentum): 16 warps per CTA, three CTAs per SM; measured on
     // configs[4] against the 256-thread shape: 0.819 -> 0.808 ms all active, 0.824 -> 0.777 ms with stragglers
-    TmaVariant{512, 3, LAYUP_TMA_TABLE(false, 512, 3), LAYUP_TMA_TABLE(true, 512, 3)},
+    TmaVariant{512, 3, 0, 0, LAYUP_TMA_TABLE(false, 512, 3, 0, 1), LAYUP_TMA_TABLE(true, 512, 3, 0, 1)},
+    // split staging, five CTAs per SM: the last array (m, or AdamW's v) through registers.  The straggler-mode
+    // default when the optimiser has state: configs[2] shapes with 25 % stragglers 13.56 -> 12.92 ms
+    TmaVariant{256, 5, 1, 4, LAYUP_TMA_TABLE(false, 256, 5, 1, 4), LAYUP_TMA_NONE},
 };
-constexpr int kTmaBigTile = 4;
+constexpr int kTmaBigTile = 4, kTmaSplit = 5;
 constexpr int kNumTma = sizeof(kTma) / sizeof(kTma[0]);
 
 }  // namespace
 
 int tma_num_variants() { return kNumTma; }
 int tma_default_variant(int n_items, int n_sections) { return (n_items >= 2048 && n_sections == 2) ? kTmaBigTile : 0; }
-
-size_t tma_smem_bytes(int K, int C, int opt, bool fused) {
+// straggler mode, optimiser with state: the thread shape of the launches that are not latency bound (-1: none)
+int tma_split_variant(int n_items, int n_sections) {
+  return n_sections >= 3 && n_items <= kTma[kTmaSplit].items * kTma[kTmaSplit].threads ? kTmaSplit : -1;
+}
+int tma_variant_rega(int variant, int opt) {
   const int narr = opt == OPT_ADAMW ? 4 : opt == OPT_SGD_MOM ? 3 : 2;
-  size_t b = (size_t)K * C * sizeof(float4) * narr + 8;                        // staged arrays + mbarrier
+  const int r = variant >= 0 && variant < kNumTma ? kTma[variant].rega : 0;
+  return r < narr ? r : narr - 1;
+}
+int tma_variant_max_items(int variant) {
+  return variant >= 0 && variant < kNumTma && kTma[variant].rega > 0 ? kTma[variant].items * kTma[variant].threads : 0;
+}
+
+size_t tma_smem_bytes(int K, int C, int opt, bool fused, int rega, bool gather4) {
+  const int narr = (opt == OPT_ADAMW ? 4 : opt == OPT_SGD_MOM ? 3 : 2) - rega;
+  size_t b = (size_t)(gather4 ? (K + 3) / 4 * 4 : K) * C * sizeof(float4) * narr + 8;   // staged arrays (gather4: whole groups of four rows) + mbarrier
   if (fused) b += sizeof(double) * K * (opt == OPT_ADAMW ? 4 : 2) + sizeof(int) * K;   // wh, wnew (, beta powers), peer
   b += sizeof(int) * 3 * (size_t)K + sizeof(float) * K * (opt == OPT_ADAMW ? 3 : 1) + (size_t)K;
+  b += 4;                                                                      // flags padded to whole groups of four
   return b;
 }
 
-bool tma_has_fused(int variant) { return variant >= 0 && variant < kNumTma && kTma[variant].fused[0][0] != nullptr; }
+bool tma_has_fused(int variant) { return variant >= 0 && variant < kNumTma && kTma[variant].fused[0][0][0] != nullptr; }
 
-cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_bytes, int *threads, int *ctas_per_sm) {
+cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, bool strag, int smem_bytes, int *threads, int *ctas_per_sm) {
   if (variant < 0 || variant >= kNumTma || opt < 0 || opt > 2) return cudaErrorInvalidValue;
   const TmaVariant &v = kTma[variant];
   cudaError_t e;
   int occ = 1 << 30;
-  for (TmaFn f : {v.fn[opt][symmetric ? 1 : 0], v.fused[opt][symmetric ? 1 : 0]}) {
+  for (TmaFn f : {v.fn[strag ? 1 : 0][opt][symmetric ? 1 : 0], v.fused[strag ? 1 : 0][opt][symmetric ? 1 : 0]}) {
     if (!f) continue;
     if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
@@ -375,7 +484,7 @@ cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, int smem_byte
 cudaError_t launch_update_tma(const UpdateParams &p, const PosTable &tab, int variant, bool fused, bool pdl, int grid,
                               int smem_bytes, cudaStream_t s) {
   const TmaVariant &v = kTma[variant];
-  TmaFn f = (fused ? v.fused : v.fn)[p.opt][p.symmetric ? 1 : 0];
+  TmaFn f = (fused ? v.fused : v.fn)[p.all_active ? 0 : 1][p.opt][p.symmetric ? 1 : 0];
   if (!f) return cudaErrorInvalidValue;
   // two-launch path: behind the schedule kernel, programmatic stream serialization lets this kernel's
   // prologue and tile loads overlap it (griddepcontrol.wait above guards the tables);
