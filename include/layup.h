@@ -97,7 +97,7 @@ typedef struct {
                            default)                                                                  */
   int32_t stages;       /* persistent shape: depth of the TMA ring; default: as deep as fits        */
   int32_t group_threads;/* persistent shape: threads per consumer group (multiple of 32); default
-                           512 with one group, 256 with more                                        */
+                           512 with one group (768 for tiles of 2048+ items), 256 with more         */
 } layup_tuning;
 
 typedef struct {

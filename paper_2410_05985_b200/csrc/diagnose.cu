@@ -36,10 +36,6 @@ struct DiagParams {
   int32_t stages;          // ring depth (ring kernel); 1 or 2 (general kernel)
 };
 
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
@@ -348,7 +344,7 @@ cudaError_t diag_plan(int K, size_t smem_optin, int *C, int *stages, int *smem_b
     // as deep as fits in the ~224 KB of shared memory of the SM's one CTA
     const size_t budget = (size_t)(224 * 1024) - 1024 - sizeof(double) * r->ncw * r->kt;
     int S = (int)((budget < smem_optin ? budget : smem_optin) / ((size_t)K * tf * sizeof(float) + 16));
-    if (S > 8) S = 8;
+    if (S > 14) S = 14;
     if (S >= 2) {
       *C = tf / 4;
       *stages = S;

@@ -42,9 +42,6 @@ constexpr int kPsMaxConsumers = 768;                  // consumer threads per CT
 constexpr int kPsMaxThreads = kPsMaxConsumers + 32 * kPsProducers;
 constexpr int kPsMaxEntries = 4;                      // table entries per producer lane: K <= 128
 
-__device__ __forceinline__ void ps_arrive(uint64_t *bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
 __device__ __forceinline__ void group_barrier(int group, int threads) {
   asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(threads) : "memory");
 }
@@ -128,7 +125,7 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
           t = sentinels == 0 ? (long long)(unsigned)atomicAdd(p.ps_ticket, 1) : n_tiles;
           if (t >= n_tiles) t = -1;
           tile_of[s] = t;
-          ps_arrive(sched + s);                            // release: the other producer warps may read it
+          mbar_arrive(sched + s);                            // release: the other producer warps may read it
         }
         tile = __shfl_sync(0xFFFFFFFFu, t, 0);
       } else {
@@ -140,7 +137,7 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
       if (tile < 0) {
         // one end marker per consumer group (consecutive iterations belong to different groups)
         __syncwarp();
-        if (lane == 0) ps_arrive(full + s * NARR);
+        if (lane == 0) mbar_arrive(full + s * NARR);
         if (++sentinels == G) return;
         if (++s == S) { s = 0; ph ^= 1u; }
         continue;
@@ -271,7 +268,7 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
     // every thread of the group is past its reads of g, m, v: those slots go back to the producers now
     if ((tid & 31) == 0) {
 #pragma unroll
-      for (int a = 1; a < NARR; ++a) ps_arrive(empty + s * NARR + a);
+      for (int a = 1; a < NARR; ++a) mbar_arrive(empty + s * NARR + a);
     }
     if (SYM) {
       // ---- phase 2 (symmetric): every scalar column runs the K exchanges in worker order
@@ -297,7 +294,7 @@ __global__ void __launch_bounds__(kPsMaxThreads, 1)
     }
     fence_proxy_async();   // the x slot was written through the generic proxy; the TMA engine refills it next
     __syncwarp();
-    if ((tid & 31) == 0) ps_arrive(empty + s * NARR);     // this warp is done with the stage
+    if ((tid & 31) == 0) mbar_arrive(empty + s * NARR);     // this warp is done with the stage
     s += G;
     if (s >= S) { s -= S; ph ^= 1u; }
   }
@@ -347,7 +344,8 @@ void persist_shape(int *stages, int n_items, int want_groups, int want_gs, int *
   int g = want_groups > 0 ? want_groups : (*stages >= 4 ? 2 : 1);
   while (g > 1 && *stages / g < 2) --g;
   *stages -= *stages % g;
-  int t = want_gs > 0 ? want_gs : (g == 1 ? 512 : 256);
+  // one group: 512 threads, 768 for tiles of >= 2048 items (configs[4], K = 64: 0.859 -> 0.826 ms)
+  int t = want_gs > 0 ? want_gs : (g == 1 ? (n_items >= 2048 ? 768 : 512) : 256);
   t = t / 32 * 32;
   if (t < 32) t = 32;
   while (t > 32 && (t * g > kPsMaxConsumers || t > n_items)) t -= 32;
