@@ -85,7 +85,8 @@ typedef struct {
                            table (0 = the library's choice; 1 128 threads x 8 CTAs/SM, 2 512 x 2,
                            3 256 x 2, 4 512 x 3, 5 256 x 5 with the last array of x, g, m, v staged
                            through registers instead of shared memory -- what straggler-mode launches
-                           take by default when the optimiser has state);
+                           take by default when the optimiser has state, 6 256 x 6 -- the default for
+                           SGD without momentum and tiles of <= 1024 items);
                            persistent shape: consumer groups per CTA (0 = as many as the ring feeds) */
   int32_t ctas_per_sm;  /* cap on resident CTAs per SM of persistent grids; default: all that fit   */
   int32_t pdl;          /* 0 auto = 1; 1: the update kernel is a programmatic dependent launch behind

@@ -35,7 +35,7 @@ struct layup_ctx {
   int variant = 0, threads = 256;
   int rega = 0;                                        // arrays the thread shape stages through registers
   bool straggler_mode = false;                         // skip_prob > 0 or a delay-mode straggler
-  int split_variant = -1, split_smem = 0;              // straggler mode: thread shape of the non-fused launches (-1: ctx->variant)
+  int split_variant = -1, split_smem = 0;              // thread shape of the launches that are not latency bound (-1: ctx->variant)
   bool persistent = false;                             // tuning.launch_shape == 2
   int engine = 1;                                      // 1: TMA-staged kernel, 0: LDG kernel
   int32_t delay_replica = 0, delay_rounds = 0;
@@ -287,14 +287,15 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   }
   if (ctx->engine == 1) {
     CU_TRY_INIT(tma_kernel_setup(ctx->variant, ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->straggler_mode, ctx->smem, &ctx->threads, &ctx->ctas_per_sm));
-    // Straggler mode with optimiser state: launches that are not latency bound take the split-staged
-    // shape (last array through registers, five CTAs per SM)
-    if (tune.variant == 0 && ctx->straggler_mode) {
-      ctx->split_variant = tma_split_variant(K * C, ctx->n_sections);
+    // Launches that are not latency bound may take a thread shape of their own: split
+    // staging (last array through registers, five CTAs per SM) in straggler mode with optimiser
+    // state, six CTAs per SM for two-array tiles of <= 1024 items
+    if (tune.variant == 0) {
+      ctx->split_variant = tma_bulk_variant(K * C, ctx->n_sections, ctx->straggler_mode);
       if (ctx->split_variant >= 0) {
         int thr = 0, occ = 0;
         ctx->split_smem = (int)tma_smem_bytes(K, C, ctx->opt, false, tma_variant_rega(ctx->split_variant, ctx->opt), want_g4);
-        CU_TRY_INIT(tma_kernel_setup(ctx->split_variant, ctx->opt, ctx->mix_mode == kMixSymmetric, true, ctx->split_smem, &thr, &occ));
+        CU_TRY_INIT(tma_kernel_setup(ctx->split_variant, ctx->opt, ctx->mix_mode == kMixSymmetric, ctx->straggler_mode, ctx->split_smem, &thr, &occ));
       }
     }
   } else {

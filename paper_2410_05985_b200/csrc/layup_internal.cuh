@@ -113,7 +113,7 @@ size_t update_smem_bytes(int K, int C);
 // update_tma.cu -- TMA-bulk staged variants
 int tma_num_variants();
 int tma_default_variant(int n_items, int n_sections);
-int tma_split_variant(int n_items, int n_sections);
+int tma_bulk_variant(int n_items, int n_sections, bool straggler_mode);
 size_t tma_smem_bytes(int K, int C, int opt, bool fused, int rega, bool gather4);
 int tma_variant_rega(int variant, int opt);        // arrays this thread shape stages through registers
 int tma_variant_max_items(int variant);            // ... and the largest tile it takes (0 = any)

@@ -431,17 +431,23 @@ const TmaVariant kTma[] = {
     // split staging, five CTAs per SM: the last array (m, or AdamW's v) through registers.  The straggler-mode
     // default when the optimiser has state: configs[2] shapes with 25 % stragglers 13.56 -> 12.92 ms
     TmaVariant{256, 5, 1, 4, LAYUP_TMA_TABLE(false, 256, 5, 1, 4), LAYUP_TMA_NONE},
+    // two staged arrays (SGD without momentum) and tiles of <= 1024 items (K <= 16): 32 KB per CTA, so six CTAs
+    // fit per SM where the 64-register shape above stops at four (128 KB in flight per SM)
+    TmaVariant{256, 6, 0, 0, LAYUP_TMA_TABLE(false, 256, 6, 0, 1), LAYUP_TMA_NONE},
 };
-constexpr int kTmaBigTile = 4, kTmaSplit = 5;
+constexpr int kTmaBigTile = 4, kTmaSplit = 5, kTmaSix = 6;
 constexpr int kNumTma = sizeof(kTma) / sizeof(kTma[0]);
 
 }  // namespace
 
 int tma_num_variants() { return kNumTma; }
 int tma_default_variant(int n_items, int n_sections) { return (n_items >= 2048 && n_sections == 2) ? kTmaBigTile : 0; }
-// straggler mode, optimiser with state: the thread shape of the launches that are not latency bound (-1: none)
-int tma_split_variant(int n_items, int n_sections) {
-  return n_sections >= 3 && n_items <= kTma[kTmaSplit].items * kTma[kTmaSplit].threads ? kTmaSplit : -1;
+// the thread shape of the launches that are not latency bound, where it differs from the default (-1: it does not):
+// straggler mode with optimiser state -> split staging; two arrays and small tiles -> six CTAs per SM
+int tma_bulk_variant(int n_items, int n_sections, bool straggler_mode) {
+  if (straggler_mode && n_sections >= 3 && n_items <= kTma[kTmaSplit].items * kTma[kTmaSplit].threads) return kTmaSplit;
+  if (n_sections == 2 && n_items <= 1024) return kTmaSix;
+  return -1;
 }
 int tma_variant_rega(int variant, int opt) {
   const int narr = opt == OPT_ADAMW ? 4 : opt == OPT_SGD_MOM ? 3 : 2;
