@@ -86,7 +86,8 @@ typedef struct {
                            3 256 x 2, 4 512 x 3, 5 256 x 5 with the last array of x, g, m, v staged
                            through registers instead of shared memory -- what straggler-mode launches
                            take by default when the optimiser has state, 6 256 x 6 -- the default for
-                           SGD without momentum and tiles of <= 1024 items);
+                           SGD without momentum and tiles of <= 1024 items, 7 512 x 3 with the same
+                           split staging for tiles of 2048 items);
                            persistent shape: consumer groups per CTA (0 = as many as the ring feeds) */
   int32_t ctas_per_sm;  /* cap on resident CTAs per SM of persistent grids; default: all that fit   */
   int32_t pdl;          /* 0 auto = 1; 1: the update kernel is a programmatic dependent launch behind

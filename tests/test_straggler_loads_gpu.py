@@ -68,7 +68,8 @@ def _check(K, skip, mu, opt, mix, tuning, rounds=4, delay=(0, 0), per_layer=Fals
 @pytest.mark.parametrize("K,skip,mu,opt,mix", [
     (2, 0.5, 0.0, OPT_SGD, MIX_PUSHSUM), (5, 0.25, 0.9, OPT_SGD, MIX_PUSHSUM), (8, 0.25, 0.9, OPT_SGD, MIX_LOSSY),
     (16, 0.25, 0.9, OPT_SGD, MIX_PUSHSUM), (16, 0.6, 0.0, OPT_ADAMW, MIX_PUSHSUM), (33, 0.25, 0.0, OPT_SGD, MIX_SYMMETRIC),
-    (64, 0.25, 0.0, OPT_SGD, MIX_PUSHSUM), (63, 0.9, 0.9, OPT_SGD, MIX_SYMMETRIC), (100, 0.25, 0.0, OPT_ADAMW, MIX_LOSSY)])
+    (64, 0.25, 0.0, OPT_SGD, MIX_PUSHSUM), (63, 0.9, 0.9, OPT_SGD, MIX_SYMMETRIC), (100, 0.25, 0.0, OPT_ADAMW, MIX_LOSSY),
+    (32, 0.25, 0.9, OPT_SGD, MIX_PUSHSUM), (64, 0.4, 0.9, OPT_SGD, MIX_LOSSY)])
 def test_straggler_rows_by_copy_and_by_gather4(K, skip, mu, opt, mix, tma2d):
     """Two-launch path (fused = never, so the grouped kernel reads the device tables) and the default."""
     assert _check(K, skip, mu, opt, mix, dict(tma2d=tma2d, fused=FUSED_NEVER))
@@ -83,6 +84,16 @@ def test_split_staging_last_array_through_registers(K, skip, mu, opt, mix, tma2d
     """Thread shape 5 forced for every launch, with and without idle replicas, every optimiser (SGD
     without momentum stages g through registers, momentum m, AdamW v)."""
     _check(K, skip, mu, opt, mix, dict(variant=SPLIT, tma2d=tma2d))
+
+
+@pytest.mark.parametrize("K,skip,mu,variant", [(4, 0.0, 0.0, 0), (16, 0.0, 0.0, 0), (16, 0.0, 0.0, 6), (9, 0.3, 0.0, 6),
+                                               (32, 0.0, 0.9, 7), (64, 0.25, 0.9, 7), (48, 0.25, 0.9, 7)])
+def test_thread_shapes_of_the_launches_that_are_not_latency_bound(K, skip, mu, variant):
+    """Shape 6 (six CTAs per SM; the default for SGD without momentum and tiles of <= 1024 items) and
+    shape 7 (split staging for tiles of 2048 items; the straggler-mode default for K >= 32 with
+    momentum), as the library picks them (variant 0, two-launch path) and forced."""
+    _check(K, skip, mu, OPT_SGD, MIX_PUSHSUM, dict(variant=variant, fused=FUSED_NEVER))
+    _check(K, skip, mu, OPT_SGD, MIX_SYMMETRIC, dict(variant=variant, fused=FUSED_NEVER), rounds=2)
 
 
 def test_split_staging_refuses_tiles_it_cannot_hold():
