@@ -95,8 +95,8 @@ typedef struct {
   int32_t tma2d;        /* 0 auto (by K and optimiser); 1: tensor-map loads -- one 2-D tiled
                            TMA load per array and tile, and in straggler mode (skip_prob > 0 or a delay
                            straggler) tile::gather4 requests of four replica rows each; 2: 1-D bulk
-                           copies, one per (replica, array) row the round needs (the straggler-mode
-                           default)                                                                  */
+                           copies, one per (replica, array) row the round needs (what auto takes in
+                           straggler mode unless a row is only 128 B long, K >= 128)                */
   int32_t stages;       /* persistent shape: depth of the TMA ring; default: as deep as fits        */
   int32_t group_threads;/* persistent shape: threads per consumer group (multiple of 32); default
                            512 with one group (768 for tiles of 2048+ items), 256 with more         */

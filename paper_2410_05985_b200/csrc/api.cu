@@ -263,10 +263,11 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   }
   ctx->engine = tune.engine == 2 ? 0 : 1;
   ctx->straggler_mode = ctx->skip_thr != 0u || ctx->delay_rounds != 0;     // some replicas may idle in a round
-  // Straggler mode fetches exactly the rows a round needs.  tma2d = 1 asks for tile::gather4 requests
-  // (four rows each); measured on B200 it does not beat row-by-row bulk copies, which
-  // stay the default.
-  const bool want_g4 = ctx->straggler_mode && tune.launch_shape != 2 && tune.tma2d == 1 && C * 4 <= 256;
+  // Straggler mode fetches exactly the rows a round needs: row-by-row bulk copies, or tile::gather4
+  // requests of four rows each.  Measured on B200 the two tie while a row is >= 256 B
+  // and gather4 wins once rows shrink to 128 B (K >= 128: up to 18 %), so auto takes it there.
+  const bool want_g4 = ctx->straggler_mode && tune.launch_shape != 2 && C * 4 <= 256 &&
+                       (tune.tma2d == 1 || (tune.tma2d == 0 && C <= 8));
   ctx->persistent = tune.launch_shape == 2;
   ctx->variant = (ctx->persistent && tune.engine != 2) ? 0 : tune.variant;   // persistent TMA shape: variant = consumer groups
   ctx->pdl = tune.pdl != 2;

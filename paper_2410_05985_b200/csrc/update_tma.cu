@@ -143,15 +143,41 @@ __global__ void __launch_bounds__(THREADS, MINB)
   // of a replica that is active or receives, g / m / v of an active one (an idle replica costs no
   // bytes).  Every thread posts the bytes of its own copies on the barrier, and every warp arrives
   // once its lanes have posted, so the phase cannot complete before the last byte count is known.
+  // With the one-row tensor maps (layup_tuning.tma2d = 1) the same rows go out four at a time as
+  // tile::gather4 requests: slot c = (group q of four consecutive replicas, array a); a row the round
+  // does not need gets the row index K, which does not exist: no HBM traffic, zeros in shared memory
+  // (never read), and the four-row byte count still completes on the barrier.
   bool rows_issued = false;
   auto issue_rows = [&](auto flag_of) {
-    for (int c = slot0; c < K * NS; c += THREADS) {
-      const int i = c / NS, a = c - i * NS;
-      const int f = flag_of(i);
-      if (!f || (a > 0 && !(f & kFlagActive))) continue;
-      const float *src = (a == 0 ? xb : a == 1 ? gb : a == 2 ? mb : vb) + (long long)i * pad;
-      mbar_post_tx(bar, chunk);
-      bulk_g2s(xs + a * arr_items + (i << log2C), src, chunk, bar);
+    if (p.tmaps_g4 != nullptr) {
+      const int n_groups = (K + 3) >> 2;
+      const unsigned char *tm = reinterpret_cast<const unsigned char *>(p.tmaps_g4);
+      for (int c = slot0; c < n_groups * NS; c += THREADS) {
+        const int q = c / NS, a = c - q * NS;
+        int r4[4];
+        bool any = false;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int i = 4 * q + j;
+          const int f = i < K ? flag_of(i) : 0;
+          const bool need = a == 0 ? f != 0 : (f & kFlagActive) != 0;
+          r4[j] = need ? i : K;
+          any |= need;
+        }
+        if (!any) continue;
+        mbar_post_tx(bar, 4u * (uint32_t)C * 16u);
+        tma_gather4(xs + a * arr_items + ((4 * q) << log2C), tm + ((size_t)a * p.L + layer) * 128, (int)(col0 << 2),
+                    r4[0], r4[1], r4[2], r4[3], bar);
+      }
+    } else {
+      for (int c = slot0; c < K * NS; c += THREADS) {
+        const int i = c / NS, a = c - i * NS;
+        const int f = flag_of(i);
+        if (!f || (a > 0 && !(f & kFlagActive))) continue;
+        const float *src = (a == 0 ? xb : a == 1 ? gb : a == 2 ? mb : vb) + (long long)i * pad;
+        mbar_post_tx(bar, chunk);
+        bulk_g2s(xs + a * arr_items + (i << log2C), src, chunk, bar);
+      }
     }
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(bar);
@@ -261,9 +287,9 @@ __global__ void __launch_bounds__(THREADS, MINB)
     // on the stream is still running (its tile loads above do not depend on it); the tables do.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     const size_t row = (size_t)layer * K;
-    if (STRAG && p.tmaps_g4 == nullptr) {
-      // every copy depends on ONE flag only: read it straight from the device table and issue, without
-      // waiting for the tables to be staged in shared memory
+    if (STRAG) {
+      // every copy depends on one flag (four for a gather4 request) only: read them straight from the
+      // device table and issue, without waiting for the tables to be staged in shared memory
       issue_rows([&](int i) { return (int)p.t.flags[row + i]; });
       rows_issued = true;
     }
@@ -283,29 +309,7 @@ __global__ void __launch_bounds__(THREADS, MINB)
   }
 
   if (STRAG) {
-    if (p.tmaps_g4 != nullptr) {
-      // tile::gather4: request slot c = (group q of four consecutive replicas, array a); a row the
-      // round does not need gets the row index K, which does not exist: no HBM traffic, zeros in
-      // shared memory (never read)
-      const int n_groups = (K + 3) >> 2;
-      const unsigned char *tm = reinterpret_cast<const unsigned char *>(p.tmaps_g4);
-      for (int c = slot0; c < n_groups * NS; c += THREADS) {
-        const int q = c / NS, a = c - q * NS;
-        const uint32_t f4 = *reinterpret_cast<const uint32_t *>(s_flags + 4 * q);     // flags of replicas 4q .. 4q+3
-        const uint32_t need = a == 0 ? (f4 | (f4 >> 1)) & 0x01010101u : f4 & 0x01010101u;   // kFlagActive = 1, kFlagRecv = 2
-        if (need == 0u) continue;
-        int r4[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) r4[j] = (need >> (8 * j)) & 1u ? 4 * q + j : K;
-        mbar_post_tx(bar, 4u * (uint32_t)C * 16u);
-        tma_gather4(xs + a * arr_items + ((4 * q) << log2C), tm + ((size_t)a * p.L + layer) * 128, (int)(col0 << 2),
-                    r4[0], r4[1], r4[2], r4[3], bar);
-      }
-      __syncwarp();
-      if ((tid & 31) == 0) mbar_arrive(bar);
-    } else if (!rows_issued) {
-      issue_rows([&](int i) { return (int)s_flags[i]; });
-    }
+    if (!rows_issued) issue_rows([&](int i) { return (int)s_flags[i]; });   // single-launch path: the flags were computed here
     if (RA > 0) reg_loads();
   }
   mbar_wait(bar, 0);
