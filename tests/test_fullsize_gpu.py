@@ -35,9 +35,14 @@ def _hbm_or_skip(w, sections):
 
 
 # ---------------------------------------------------------------- whole-layer parity, full size
-@pytest.mark.parametrize("name,rounds", [("gpt2s_k8", 2), ("manysmall_k64", 2)])
-def test_every_element_of_every_layer_full_size(name, rounds):
+@pytest.mark.parametrize("name,rounds,skip", [("gpt2s_k8", 2, None), ("manysmall_k64", 2, None),
+                                              ("gpt2s_k8", 2, 0.25), ("manysmall_k64", 2, 0.25)])
+def test_every_element_of_every_layer_full_size(name, rounds, skip):
+    """skip = 0.25: the same shapes in straggler mode (configs[3] semantics, `bench.py --skip-prob 0.25`),
+    i.e. the straggler-mode kernels (row loads from the device flags, split staging) at full size."""
     w = synth.workload(name)
+    if skip is not None:
+        w = synth.shrink(w, w.numel, skip_prob=skip)
     _hbm_or_skip(w, 3)
     lu = LayUp(w.K, w.numel, w.lr, w.momentum, w.seed, w.peer_mode, w.skip_prob)
     ref = oracle.Oracle(w.numel, w.K, w.lr, w.momentum, w.seed, w.peer_mode, w.skip_prob)
@@ -61,7 +66,9 @@ def test_every_element_of_every_layer_full_size(name, rounds):
                 assert np.array_equal(_bits(gm), _bits(ref.m[l])), (name, step, l, "m")
         assert np.array_equal(lu.layup_weights(), ref.w)
     assert total == rounds * w.K * w.params_per_replica
-    print("%s: %d elements compared bit for bit over %d rounds" % (name, total, rounds))
+    if skip is not None:
+        assert not all(oracle.schedule(w.seed, s, w.L, w.K, w.peer_mode, w.skip_prob)[1].all() for s in range(rounds))
+    print("%s (skip %s): %d elements compared bit for bit over %d rounds" % (name, skip, total, rounds))
     lu.close()
     del lu
     torch.cuda.empty_cache()
