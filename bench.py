@@ -370,6 +370,25 @@ def per_config_report(args, rank, local_rank, barrier, main_name, main_entry):
                 out.append(config_entry(w, mode, r))
             except Exception as ex:                      # e.g. not enough HBM next to the main arena
                 out.append({"workload": w.name, "mode": mode, "error": str(ex)[:200]})
+    # straggler rounds at HBM size: configs[3]'s semantics (each replica idles with probability 0.25 per
+    # round and still receives) on the shapes of configs[1], [4] and, if a second
+    # arena fits beside the main one, configs[2]
+    for name in ("gpt2s_k8", "manysmall_k64", "gpt2m_k16"):
+        w = synth.shrink(synth.workload(name), synth.workload(name).numel, skip_prob=0.25)
+        need = w.K * sum((n + 31) // 32 * 32 for n in w.numel) * 4 * 3 + (6 << 30)
+        if torch.cuda.mem_get_info()[0] < need:
+            out.append({"workload": "%s shapes, skip_prob 0.25" % name, "mode": "round", "error": "needs %.0f GB of free HBM" % (need / 2**30)})
+            continue
+        try:
+            t = Timed(args, w, rank, local_rank, "round", barrier)
+            r = t.run(10, max(args.warmup, 3))
+            t.close()
+            e = config_entry(w, "round", r)
+            e["workload"] = "%s shapes, skip_prob 0.25" % name
+            e["note"] = "effective bytes: 12/20 B per active param-update, 8 B per element of an idle replica that receives a push"
+            out.append(e)
+        except Exception as ex:
+            out.append({"workload": "%s shapes, skip_prob 0.25" % name, "mode": "round", "error": str(ex)[:200]})
     return out
 
 

@@ -8,7 +8,7 @@
  * ("Local Update"), then the push-sum gossip mix of that copy into a
  * randomly chosen peer's copy of the same layer ("Peer Update",
  * PAPER.md:104-106 weights), with no buffer or queue.  The
- * deterministic reading of the paper's racy system is DESIGN.md "Readings" R1-R23.
+ * deterministic reading of the paper's racy system is DESIGN.md "Readings" R1-R25.
  *
  * Conventions
  *  - All functions return int: LAYUP_OK (0) or a negative LAYUP_E* code; no exceptions,
