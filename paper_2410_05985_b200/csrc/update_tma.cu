@@ -9,19 +9,21 @@
 //   - all active but no tensor map (K > 256, huge slices): K x arrays 1-D bulk copies (cp.async.bulk,
 //     SASS UBLKCP), spread over all warps;
 //   - straggler mode (STRAG): the rows a round needs -- x of every replica that is active or
-//     receives, g / m / v of the active ones -- are only known on the device.  They are fetched in
-//     groups of four consecutive replicas with cp.async.bulk.tensor.2d.tile::gather4 (SASS
-//     UTMALDG.2D.GATHER4: four arbitrary rows of the [K][padded slice] view per request; a row the
-//     round does not need is given an out-of-range index, which costs no HBM traffic and lands as
-//     zeros), so an idle replica costs no bytes and a tile issues a quarter of the requests that
-//     row-by-row copies need.
+//     receives, g / m / v of the active ones -- are only known on the device.  Every thread reads
+//     the flag of its (replica, array) slot straight from the device table and issues that row's
+//     bulk copy at once, posting its bytes on the barrier itself (one arrival per warp): no staging
+//     of the flags, no CTA barrier in front of the loads; an idle replica costs no bytes.  With
+//     one-row tensor maps (tiles whose rows are only 128 B long, or layup_tuning.tma2d = 1) the same
+//     rows go out four at a time as cp.async.bulk.tensor.2d.tile::gather4 requests (SASS
+//     UTMALDG.2D.GATHER4; a row the round does not need is given an out-of-range index, which
+//     costs no HBM traffic and lands as zeros).
 // The local step then runs out of shared memory, y overwrites x in place (the "send" is an
 // on-chip read), m' (and AdamW's v') go straight to HBM, and after one CTA barrier
 // every receiver folds its senders and writes x once.  HBM traffic: 12 B (SGD) / 20 B (momentum) /
 // 28 B (AdamW) per parameter update, nothing read or written twice.
 // Template parameters: OPT = local optimiser (rule.cuh), SYM = symmetric pairwise averaging
 // instead of the push-sum fold, FUSED = the schedule stage runs in this kernel (one launch),
-// STRAG = the ctx has a straggler mode (some replicas may idle: compacted rows),
+// STRAG = the ctx has a straggler mode (some replicas may idle in a round),
 // REGA / U = split staging (below).
 #include "layup_internal.cuh"
 #include "philox.cuh"
@@ -32,11 +34,6 @@ namespace layup {
 
 namespace {
 
-// FUSED: the schedule stage (schedule.cu) runs inside this kernel -- ONE launch per round or
-// per layer event instead of two.  Every CTA of a layer recomputes that layer's O(K) schedule in
-// shared memory from the same inputs (seed, step, w, beta powers), so all CTAs agree bit for bit;
-// the CTA that is LAST to have read the state (a ticket per layer) writes the new w / beta powers
-// back in place.  Used for launches of few tiles (launch-latency bound) and K <= kFusedMaxK.
 __device__ __forceinline__ float4 ld4_stream(const float *p) {   // read once, by this thread only: keep it out of L1
   float4 v;
   asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
@@ -44,6 +41,12 @@ __device__ __forceinline__ float4 ld4_stream(const float *p) {   // read once, b
   return v;
 }
 
+// FUSED: the schedule stage (schedule.cu) runs inside this kernel -- ONE launch per round or
+// per layer event instead of two.  Every CTA of a layer recomputes that layer's O(K) schedule in
+// shared memory from the same inputs (seed, step, w, beta powers), so all CTAs agree bit for bit;
+// the CTA that is LAST to have read the state (a ticket per layer) writes the new w / beta powers
+// back in place.  Used for launches of few tiles (launch-latency bound) and K <= kFusedMaxK.
+//
 // REGA / U: split staging.  Only x has to be in shared memory (it becomes y, which the receivers
 // of other replicas read); g, m and v are consumed once, by the thread that takes the local step
 // of that element.  REGA > 0 brings the LAST REGA arrays of (x, g, m, v) into REGISTERS with plain
