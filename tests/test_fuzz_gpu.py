@@ -37,7 +37,7 @@ def _draw(seed):
     return cfg, big
 
 
-@pytest.mark.parametrize("case", range(60))
+@pytest.mark.parametrize("case", range(100))
 def test_random_configuration_matches_the_oracle(case):
     cfg, big = _draw(1000 + case)
     K, numel = cfg["K"], cfg["numel"]
