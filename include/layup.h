@@ -79,7 +79,7 @@ typedef struct {
                            through a multi-stage TMA ring                             */
   int32_t fused;        /* 0 auto = 1; 1: launches of at most fused_waves waves of work items run the
                            schedule stage inside the update kernel (ONE launch); 2: never            */
-  int32_t fused_waves;  /* default 4                                                                */
+  int32_t fused_waves;  /* default 4 (K <= 16), 2 (K <= 32), 1 (larger K)                            */
   int32_t tile_items;   /* float4 items (replicas x columns) per work item; default 1024            */
   int32_t variant;      /* grouped shape: thread shape of the update kernel, an index into update_tma.cu's
                            table (0 = the library's choice; 1 128 threads x 8 CTAs/SM, 2 512 x 2,

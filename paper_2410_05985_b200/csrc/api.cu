@@ -309,7 +309,9 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   //  HBM-sized rounds -- the redundant schedule stage is only free while the launch is latency bound)
   //  (K = 8 always fused: per-layer events 3.03 -> 2.97 ms per round, but AdamW rounds -0.7 % and
   //  straggler rounds -12 %, where the schedule stage sits in front of the loads: not done.)
-  const int waves = tune.fused_waves > 0 ? tune.fused_waves : 4;
+  //  (the redundant stage is O(K) per CTA: per-layer events of configs[4], K = 64, 1.005 ms per round with a
+  //  4-wave bound, 0.957 with 1 wave; configs[1], K = 8: 2.99 ms with 4 waves, 3.03 with 1 or 2)
+  const int waves = tune.fused_waves > 0 ? tune.fused_waves : (K <= 16 ? 4 : K <= 32 ? 2 : 1);
   ctx->fused_max_tiles = (long long)waves * ctx->n_sm * ctx->ctas_per_sm;
   const int cap = tune.ctas_per_sm;
   if (cap > 0 && cap < ctx->ctas_per_sm) ctx->ctas_per_sm = cap;

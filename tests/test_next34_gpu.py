@@ -226,7 +226,7 @@ def test_single_launch_path_equals_two_launch_path(opt, mix, mu, skip, K):
     kw = ADAM if opt == OPT_ADAMW else {}
     outs, launches = [], []
     for fused in (FUSED_AUTO, FUSED_NEVER):
-        w, lu, ref, _ = _pair(K, NUMEL, 1e-3, mu, 31, skip, opt, mix, tuning=dict(fused=fused), **kw)
+        w, lu, ref, _ = _pair(K, NUMEL, 1e-3, mu, 31, skip, opt, mix, tuning=dict(fused=fused, fused_waves=4), **kw)
         n0 = lu.layup_launch_count()
         _run(w, lu, ref, None, 4)
         # per-layer events take the same path
