@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(CSRC, "liblayup.so")
 SOURCES = ["api.cu", "schedule.cu", "update.cu", "update_tma.cu", "update_persist.cu", "diagnose.cu"]
-HEADERS = ["layup_internal.cuh", "philox.cuh", "rule.cuh", "tma_ptx.cuh", os.path.join("..", "..", "include", "layup.h")]
+HEADERS = ["layup_internal.cuh", "philox.cuh", "rule.cuh", "schedule_body.cuh", "tma_ptx.cuh", os.path.join("..", "..", "include", "layup.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "--threads", "0", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
 
