@@ -489,6 +489,20 @@ def run_ours(args, w, rank, world, local_rank):
             e2e = {"value": world * sum(e_ups) / e_s, "unit": UNIT, "h2d_bytes_per_step": 4 * total,
                    "d2h_bytes_per_step": 4 * total, "steps": args.e2e_steps, "ms_per_step": e_s / args.e2e_steps * 1e3,
                    "api": "layup_round_host (pinned host grads in, params out, layer-pipelined)"}
+            # the same call when the step's result read back is a metric, not the parameters: gradients in,
+            # the push-sum weights w[L][K] out -- what a training loop would do every step
+            barrier()
+            tm0 = time.perf_counter()
+            m_first = step
+            for _ in range(args.e2e_steps):
+                lu.layup_round_host(step, g_host, None); step += 1
+                lu.layup_weights()
+            barrier()
+            m_s = time.perf_counter() - tm0
+            _, m_ups = algorithmic_bytes(w, lu, range(m_first, m_first + args.e2e_steps), args)
+            e2e["metric_only"] = {"value": world * sum(m_ups) / m_s, "unit": UNIT, "h2d_bytes_per_step": 4 * total,
+                                  "d2h_bytes_per_step": 8 * w.L * w.K, "ms_per_step": m_s / args.e2e_steps * 1e3,
+                                  "api": "layup_round_host (pinned host grads in, no parameter read-back) + layup_weights"}
             del g_host, x_host
         except Exception as ex:                  # e.g. the box cannot pin 2 x K x N x 4 bytes
             e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
