@@ -46,13 +46,15 @@ __device__ __forceinline__ double warp_sum(double v) {
 // NCW: consumer warps; a thread owns ONE scalar column of the tile (tile row = NCW*32 floats)
 // kDiagProducers producer warps share a tile's row copies (a warp issues its bulk copies one lane at a time)
 // KEEP: keep the converted tile in registers between the two passes (one fp32->fp64 conversion per element)
+// CPT: scalar columns per consumer thread (columns tid, tid + NC, ...): for K <= 8 two columns per thread
+//      make the tile as large (32 KB) and the per-tile barrier traffic as rare as at K = 16
 constexpr int kDiagProducers = 4;
-template <int KT, bool KEEP, int NCW>
+template <int KT, bool KEEP, int NCW, int CPT = 1>
 __global__ void __launch_bounds__(NCW * 32 + 32 * kDiagProducers, 1)
     layup_disagreement_kernel(const __grid_constant__ DiagParams p, const __grid_constant__ PosTable tab) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int NC = NCW * 32;                                           // consumer threads
-  constexpr int TF = NC;                                                 // floats per replica row of a tile
+  constexpr int TF = NC * CPT;                                           // floats per replica row of a tile
   const int K = p.K, S = p.stages, tid = threadIdx.x;
   float *ring = reinterpret_cast<float *>(smem_raw);                    // [S][K][TF]
   uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)S * K * TF);   // [S]
@@ -145,34 +147,46 @@ __global__ void __launch_bounds__(NCW * 32 + 32 * kDiagProducers, 1)
     if (KEEP && K == KT && left >= TF) {
       // ---- whole tile, K == KT: no predicate anywhere; every element is converted once and kept in
       // registers for both passes, the stage is released right after the loads, and the consensus
-      // sum runs on four chains
-      double xd[KT], m4[4] = {0.0, 0.0, 0.0, 0.0};
+      // sum of a column runs on four chains (two per column with two columns per thread)
+      constexpr int CH = CPT == 1 ? 4 : 2;
+      double xd[CPT][KT], mc[CPT][CH];
 #pragma unroll
-      for (int i = 0; i < KT; ++i) {
-        xd[i] = (double)row0[(size_t)i * TF];
-        m4[i & 3] = fma(weighted ? coef[i] : inv_k, xd[i], m4[i & 3]);
+      for (int c = 0; c < CPT; ++c) {
+#pragma unroll
+        for (int h = 0; h < CH; ++h) mc[c][h] = 0.0;
+#pragma unroll
+        for (int i = 0; i < KT; ++i) {
+          xd[c][i] = (double)row0[(size_t)i * TF + c * NC];
+          mc[c][i % CH] = fma(weighted ? coef[i] : inv_k, xd[c][i], mc[c][i % CH]);
+        }
       }
       __syncwarp();
       if ((tid & 31) == 0) mbar_arrive(empty + s);                      // the tile now lives in registers
-      const double m = (m4[0] + m4[1]) + (m4[2] + m4[3]);
 #pragma unroll
-      for (int i = 0; i < KT; ++i) {
-        const double d = xd[i] - m;
-        acc[i] = fma(d, d, acc[i]);
+      for (int c = 0; c < CPT; ++c) {
+        const double m = CH == 4 ? (mc[c][0] + mc[c][1]) + (mc[c][2] + mc[c][3]) : mc[c][0] + mc[c][1];
+#pragma unroll
+        for (int i = 0; i < KT; ++i) {
+          const double d = xd[c][i] - m;
+          acc[i] = fma(d, d, acc[i]);
+        }
       }
     } else {
       // ---- ragged tail of a layer, or K < KT: same arithmetic, predicated
-      const bool live = (long long)tid < left;                          // pads are part of the slice (zero in every replica)
-      double m = 0.0;
-      if (live) {
 #pragma unroll
-        for (int i = 0; i < KT; ++i)
-          if (i < K) m = fma(weighted ? coef[i] : inv_k, (double)row0[(size_t)i * TF], m);
+      for (int c = 0; c < CPT; ++c) {
+        const bool live = (long long)(tid + c * NC) < left;             // pads are part of the slice (zero in every replica)
+        double m = 0.0;
+        if (live) {
 #pragma unroll
-        for (int i = 0; i < KT; ++i) {
-          if (i < K) {
-            const double d = (double)row0[(size_t)i * TF] - m;
-            acc[i] = fma(d, d, acc[i]);
+          for (int i = 0; i < KT; ++i)
+            if (i < K) m = fma(weighted ? coef[i] : inv_k, (double)row0[(size_t)i * TF + c * NC], m);
+#pragma unroll
+          for (int i = 0; i < KT; ++i) {
+            if (i < K) {
+              const double d = (double)row0[(size_t)i * TF + c * NC] - m;
+              acc[i] = fma(d, d, acc[i]);
+            }
           }
         }
       }
@@ -308,17 +322,17 @@ __global__ void __launch_bounds__(kGenThreads) layup_disagreement_general(const 
 
 using DiagFn = void (*)(const DiagParams, const PosTable);
 struct RingShape {
-  int kt, ncw;
+  int kt, ncw, cpt;     // a tile row is ncw * 32 * cpt floats
   DiagFn fn;
 };
 // one CTA per SM: the registers go to the per-replica accumulators (and the fp64 copy of the tile),
 // the shared memory to a deep ring; 16 consumer warps while the accumulators allow it (8 were measured
 // issue-bound: profiles/r2_disagreement_gpt2m_k16_8warps.txt)
 const RingShape kRing[] = {
-    {8, 16, layup_disagreement_kernel<8, true, 16>},
-    {16, 16, layup_disagreement_kernel<16, true, 16>},
-    {32, 16, layup_disagreement_kernel<32, false, 16>},
-    {64, 8, layup_disagreement_kernel<64, false, 8>},
+    {8, 16, 2, layup_disagreement_kernel<8, true, 16, 2>},
+    {16, 16, 1, layup_disagreement_kernel<16, true, 16>},
+    {32, 16, 1, layup_disagreement_kernel<32, false, 16>},
+    {64, 8, 1, layup_disagreement_kernel<64, false, 8>},
 };
 const RingShape *ring_shape(int K) {
   for (const RingShape &r : kRing)
@@ -340,7 +354,7 @@ int general_iters(int K, int C) { return (K * C + kGenThreads - 1) / kGenThreads
 cudaError_t diag_plan(int K, size_t smem_optin, int *C, int *stages, int *smem_bytes, int *ctas_per_sm) {
   cudaError_t e;
   if (const RingShape *r = ring_shape(K)) {
-    const int tf = r->ncw * 32;
+    const int tf = r->ncw * 32 * r->cpt;
     // as deep as fits in the ~224 KB of shared memory of the SM's one CTA
     const size_t budget = (size_t)(224 * 1024) - 1024 - sizeof(double) * r->ncw * r->kt;
     int S = (int)((budget < smem_optin ? budget : smem_optin) / ((size_t)K * tf * sizeof(float) + 16));
@@ -370,7 +384,7 @@ cudaError_t launch_disagreement(const float *x, const double *w, double *dist, i
                                 const PosTable &tab, int grid, int smem_bytes, cudaStream_t s) {
   DiagParams p{x, w, dist, K, C, log2C, stages};
   const RingShape *r = ring_shape(K);
-  if (r && C * 4 == r->ncw * 32 && stages >= 2 && (size_t)smem_bytes == ring_smem(K, C * 4, stages, r->kt, r->ncw)) {
+  if (r && C * 4 == r->ncw * 32 * r->cpt && stages >= 2 && (size_t)smem_bytes == ring_smem(K, C * 4, stages, r->kt, r->ncw)) {
     r->fn<<<grid, r->ncw * 32 + 32 * kDiagProducers, smem_bytes, s>>>(p, tab);
     return cudaGetLastError();
   }
