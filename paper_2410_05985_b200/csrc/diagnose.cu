@@ -328,9 +328,14 @@ struct RingShape {
 // one CTA per SM: the registers go to the per-replica accumulators (and the fp64 copy of the tile),
 // the shared memory to a deep ring; 16 consumer warps while the accumulators allow it (8 were measured
 // issue-bound: profiles/r2_disagreement_gpt2m_k16_8warps.txt)
+// K <= 16: one instantiation per K, so that K == KT always takes the unpredicated path (the predicated
+// one runs at 4-5.8 TB/s where the exact one reaches 6.4-6.8); columns per thread chosen so that a
+// thread keeps about 16 converted elements
+#define LAYUP_DIAG(KT_, CPT_) {KT_, 16, CPT_, layup_disagreement_kernel<KT_, true, 16, CPT_>}
 const RingShape kRing[] = {
-    {8, 16, 2, layup_disagreement_kernel<8, true, 16, 2>},
-    {16, 16, 1, layup_disagreement_kernel<16, true, 16>},
+    LAYUP_DIAG(1, 8),  LAYUP_DIAG(2, 8),  LAYUP_DIAG(3, 4),  LAYUP_DIAG(4, 4),  LAYUP_DIAG(5, 3),  LAYUP_DIAG(6, 2),
+    LAYUP_DIAG(7, 2),  LAYUP_DIAG(8, 2),  LAYUP_DIAG(9, 1),  LAYUP_DIAG(10, 1), LAYUP_DIAG(11, 1), LAYUP_DIAG(12, 1),
+    LAYUP_DIAG(13, 1), LAYUP_DIAG(14, 1), LAYUP_DIAG(15, 1), LAYUP_DIAG(16, 1),
     {32, 16, 1, layup_disagreement_kernel<32, false, 16>},
     {64, 8, 1, layup_disagreement_kernel<64, false, 8>},
 };
