@@ -324,6 +324,7 @@ using DiagFn = void (*)(const DiagParams, const PosTable);
 struct RingShape {
   int kt, ncw, cpt;     // a tile row is ncw * 32 * cpt floats
   DiagFn fn;
+  bool exact;           // only for K == kt (its predicated path would be slower than a general shape's)
 };
 // one CTA per SM: the registers go to the per-replica accumulators (and the fp64 copy of the tile),
 // the shared memory to a deep ring; 16 consumer warps while the accumulators allow it (8 were measured
@@ -331,17 +332,23 @@ struct RingShape {
 // K <= 16: one instantiation per K, so that K == KT always takes the unpredicated path (the predicated
 // one runs at 4-5.8 TB/s where the exact one reaches 6.4-6.8); columns per thread chosen so that a
 // thread keeps about 16 converted elements
-#define LAYUP_DIAG(KT_, CPT_) {KT_, 16, CPT_, layup_disagreement_kernel<KT_, true, 16, CPT_>}
+#define LAYUP_DIAG(KT_, CPT_) {KT_, 16, CPT_, layup_disagreement_kernel<KT_, true, 16, CPT_>, false}
+// 16 < K <= 32: the converted tile still fits in registers with 8 consumer warps (K = 32: 6.2 -> 6.8 TB/s)
+#define LAYUP_DIAG8(KT_, KEEP_) {KT_, 8, 1, layup_disagreement_kernel<KT_, KEEP_, 8>, true}
 const RingShape kRing[] = {
     LAYUP_DIAG(1, 8),  LAYUP_DIAG(2, 8),  LAYUP_DIAG(3, 4),  LAYUP_DIAG(4, 4),  LAYUP_DIAG(5, 3),  LAYUP_DIAG(6, 2),
     LAYUP_DIAG(7, 2),  LAYUP_DIAG(8, 2),  LAYUP_DIAG(9, 1),  LAYUP_DIAG(10, 1), LAYUP_DIAG(11, 1), LAYUP_DIAG(12, 1),
     LAYUP_DIAG(13, 1), LAYUP_DIAG(14, 1), LAYUP_DIAG(15, 1), LAYUP_DIAG(16, 1),
-    {32, 16, 1, layup_disagreement_kernel<32, false, 16>},
-    {64, 8, 1, layup_disagreement_kernel<64, false, 8>},
+    LAYUP_DIAG8(20, true), LAYUP_DIAG8(24, true), LAYUP_DIAG8(28, true), LAYUP_DIAG8(32, true),
+    LAYUP_DIAG8(40, false), LAYUP_DIAG8(48, false), LAYUP_DIAG8(56, false),
+    {32, 16, 1, layup_disagreement_kernel<32, false, 16>, false},
+    {64, 8, 1, layup_disagreement_kernel<64, false, 8>, false},
 };
 const RingShape *ring_shape(int K) {
   for (const RingShape &r : kRing)
-    if (K <= r.kt) return &r;
+    if (K == r.kt) return &r;
+  for (const RingShape &r : kRing)
+    if (K <= r.kt && !r.exact) return &r;
   return nullptr;
 }
 
