@@ -241,6 +241,48 @@ int layup_disagreement(layup_ctx *ctx, int32_t weighted, double *dist /*[L*K]*/,
 /* Device time of the reduction kernel(s) of the last layup_disagreement call (CUDA events). */
 int layup_disagreement_ms(layup_ctx *ctx, double *ms);
 
+/* ---- the same diagnostic for callers that must not allocate device memory ------------ */
+/* Who this is for.  LayUp's per-layer events are issued from backward hooks while the backward
+ * pass and earlier layers' gossip are still running on other streams.  A
+ * monitoring hook that wants the disagreement curve of Fig. A1 from inside
+ * that window must not call cudaMalloc / cudaFree: both wait for the whole device, which would
+ * serialise exactly the overlap the method exists for.  The same holds for a job that has
+ * handed all of HBM to the arena and to a framework's caching allocator (nothing is left for a
+ * raw cudaMalloc to succeed with), and for a process that only borrows a parameter buffer in the
+ * arena layout and never created a ctx -- layup_init allocates the library's tables, so a
+ * ctx-based call is no use to it.
+ *
+ * layup_disagreement_static computes what layup_disagreement computes, with the same kernels,
+ * without a ctx and without allocating anything, on the calling thread's CURRENT device.  The
+ * accumulators the reduction kernel adds into, and the device copy of the weights, live in
+ * one array compiled into the library: 2 * LAYUP_STATIC_MAX_PAIRS doubles (256 KiB) of device
+ * memory on every GPU the process uses with this library, held from the moment the library's
+ * code is loaded on that GPU until the process exits.
+ *   x_dev    DEVICE, 128-B aligned, on the current device: one X section in the arena layout
+ *            above for (K, L, numel) -- layer l starts at sum_{l'<l} K*pad(numel[l']) floats, its
+ *            K slices pad(numel[l]) floats apart, pad(n) = n rounded up to 32, pad floats ZERO.
+ *            layup_ptr(ctx, LAYUP_WHAT_X, 0, 0) of a ctx with the same (K, numel) is such a pointer.
+ *   numel    HOST [L], each >= 1.        K in [1, LAYUP_MAX_K],  L >= 1.
+ *   w        HOST [L*K] consensus coefficients (the push-sum weights of layup_weights for the
+ *            weighted consensus), or NULL for the plain mean 1/K.
+ *   dist     HOST [L*K] output, dist[l*K+i] as in layup_disagreement.
+ * Limits and errors: L*K > LAYUP_STATIC_MAX_PAIRS, bad sizes, a misaligned x_dev or one that is
+ * not device memory of the current device give LAYUP_EINVAL before anything is enqueued (text:
+ * layup_last_error(NULL)); CUDA failures give LAYUP_ECUDA.  The call issues a memset of its
+ * accumulators, the copy of w, the kernel(s) and the read-back on `cuda_stream`, in stream order
+ * after the caller's writes to x on that stream, and returns when dist is complete (synchronous;
+ * it does NOT wait for other streams -- order the writers of x before it yourself).  It calls no
+ * cudaMalloc / cudaFree, creates no stream or event and uses no allocating library routine.
+ * First call on each device: it looks up the device address of the array (cudaGetSymbolAddress)
+ * and the SM count, once, and keeps them; make that first call outside any stream capture.
+ * Sharing: every call on a device uses the one array, which still holds the previous call's
+ * sums (each call clears the part it uses before its kernel).  Two calls that overlapped on the
+ * GPU would race on it, so the library holds a process-wide lock from the first enqueue to the
+ * final stream synchronise: calls from several host threads run one after the other. */
+#define LAYUP_STATIC_MAX_PAIRS 16384   /* (layer, replica) pairs: L*K <= this                  */
+int layup_disagreement_static(const float *x_dev, int32_t K, int32_t L, const int64_t *numel,
+                              const double *w, double *dist, void *cuda_stream);
+
 /* ---- CUDA-graph capture of launching calls ------------------------------------------ */
 /* The round number is DEVICE state (one counter per layer, read and advanced by the schedule
  * stage), not a kernel argument, so a recorded sequence of launches can be replayed for later

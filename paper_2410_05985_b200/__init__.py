@@ -6,4 +6,5 @@ include/layup.h); this package is only the thin ctypes binding.  There is no CPU
 from .binding import (ENGINE_LDG, ENGINE_TMA, FUSED_AUTO, FUSED_NEVER, SHAPE_GROUPED, SHAPE_PERSISTENT,  # noqa: F401
                       LAYUP_ECUDA, LAYUP_EINVAL, LAYUP_ESTATE, LAYUP_OK, MIX_LOSSY, MIX_PUSHSUM,  # noqa: F401
                       MIX_SYMMETRIC, OPT_ADAMW, OPT_SGD, WHAT_G, WHAT_M, WHAT_V, WHAT_X,
-                      LayUp, LayUpError, layup_arena_bytes, layup_peer, load_library)
+                      LAYUP_STATIC_MAX_PAIRS, LayUp, LayUpError, layup_arena_bytes, layup_disagreement_static, layup_peer,
+                      load_library)

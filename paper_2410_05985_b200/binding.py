@@ -52,6 +52,7 @@ EXPORTS = ["layup_arena_bytes", "layup_init", "layup_destroy", "layup_ptr", "lay
            "layup_layer_update", "layup_round", "layup_round_host", "layup_sync", "layup_peer",
            "layup_schedule", "layup_schedule_tables", "layup_last_order", "layup_trace", "layup_trace_read",
            "layup_weights", "layup_state_export", "layup_state_import", "layup_disagreement", "layup_disagreement_ms",
+           "layup_disagreement_static",
            "layup_graph_begin", "layup_graph_end", "layup_graph_launch", "layup_graph_destroy",
            "layup_profile", "layup_profile_read", "layup_launch_count", "layup_last_error"]
 
@@ -83,6 +84,7 @@ def load_library():
         "layup_state_import": [vp, vp, vp, vp],
         "layup_disagreement": [vp, i32, vp, vp],
         "layup_disagreement_ms": [vp, c.POINTER(c.c_double)],
+        "layup_disagreement_static": [vp, i32, i32, c.POINTER(i64), vp, vp, vp],
         "layup_schedule_tables": [vp, i32, c.POINTER(i64), vp, vp, vp, vp, vp],
         "layup_last_order": [vp, vp, c.POINTER(i32)],
         "layup_trace": [vp, i32],
@@ -144,6 +146,29 @@ def _stream_handle(stream, device_index=None) -> Optional[int]:
     if isinstance(stream, torch.cuda.Stream):
         return stream.cuda_stream or None
     return int(stream) or None
+
+
+def layup_disagreement_static(x_dev, K: int, numel: Sequence[int], w: Optional[np.ndarray] = None,
+                              stream=None) -> np.ndarray:
+    """layup_disagreement for callers that must not allocate device memory (include/layup.h): no ctx,
+    no cudaMalloc -- the kernel's accumulators sit in an array compiled into liblayup.so, which caps
+    len(numel) * K at LAYUP_STATIC_MAX_PAIRS.  Meant for a monitoring hook that runs while backward and
+    gossip overlap (a cudaMalloc there stalls the whole device) or for a process that only borrows an
+    X section and has no ctx.  x_dev: raw device address (int) of an X section in the arena layout on the
+    CURRENT device, e.g. LayUp.ptr(WHAT_X, 0, 0)[0]; w: [L, K] float64 consensus coefficients or None
+    for the plain mean.  Returns dist[L, K].  Synchronous; concurrent callers are serialised by the
+    library because they all share that one array."""
+    L = len(numel)
+    arr = (ctypes.c_int64 * L)(*[int(v) for v in numel])
+    wd = None if w is None else np.ascontiguousarray(w, dtype=np.float64).reshape(L, int(K))
+    d = np.empty((L, int(K)), dtype=np.float64)
+    sh = _stream_handle(stream, torch.cuda.current_device()) if torch.cuda.is_available() else None
+    _check(load_library().layup_disagreement_static(int(x_dev), int(K), L, arr, None if wd is None else wd.ctypes.data,
+                                                    d.ctypes.data, sh))
+    return d
+
+
+LAYUP_STATIC_MAX_PAIRS = 16384
 
 
 class LayUp:

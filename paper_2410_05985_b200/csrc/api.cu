@@ -121,6 +121,9 @@ static int fail(layup_ctx *ctx, int code, const char *fmt, ...) {
   return code;
 }
 
+// ctx-less entry points of other translation units (diagnose.cu) leave their text behind layup_last_error(NULL)
+void layup::note_error(const char *text) { g_err = text; }
+
 #define CU_TRY(ctx, expr)                                                                      \
   do {                                                                                         \
     cudaError_t e__ = (expr);                                                                  \

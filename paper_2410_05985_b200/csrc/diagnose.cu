@@ -407,3 +407,136 @@ cudaError_t launch_disagreement(const float *x, const double *w, double *dist, i
 }
 
 }  // namespace layup
+
+// =================================================================================================
+// layup_disagreement_static (include/layup.h): the reduction above for callers that must not
+// allocate device memory -- a monitoring hook inside the backward window (cudaMalloc / cudaFree
+// wait for the whole device and would serialise the backward/gossip overlap of PAPER.md:108-112),
+// a job whose HBM is fully handed out already, a process that only borrows an X section and
+// never made a ctx (layup_init allocates).  The kernels and their launch plan are the ones
+// layup_disagreement uses; only the home of the scratch differs:
+//   ctx path:     ctx->d_dist / ctx->d_w, cudaMalloc'ed by layup_init;
+//   static path:  g_static_scratch below, part of the library image on every device.
+// =================================================================================================
+#include <cstdarg>
+#include <cstdio>
+#include <mutex>
+
+#include "../../include/layup.h"
+
+// [0, MAX_PAIRS): the fp64 sums the kernel atomicAdds into (must be zero at launch);
+// [MAX_PAIRS, 2*MAX_PAIRS): this call's copy of the consensus coefficients w (weighted mode).
+// 256 KiB per device, for as long as the library is loaded there.  The previous call's contents
+// stay in it: every call clears / overwrites the part it is about to use, in stream order.
+static __device__ __align__(256) double g_static_scratch[2 * LAYUP_STATIC_MAX_PAIRS];
+
+namespace {
+
+// In HOST code the name g_static_scratch is only the host-side shadow of the symbol -- not an
+// address a kernel may dereference.  The real device address differs per device and comes from
+// cudaGetSymbolAddress with that device current; it is looked up once per device and kept here.
+constexpr int kStaticMaxDevices = 64;
+struct StaticDevice {
+  double *scratch = nullptr;     // device address of g_static_scratch on this device
+  int n_sm = 0;
+  size_t smem_optin = 0;
+};
+StaticDevice g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mu;           // set-up AND the whole call: all calls share the one array
+
+int static_fail(int code, const char *fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  layup::note_error(buf);
+  return code;
+}
+#define STATIC_CU(expr)                                                                          \
+  do {                                                                                           \
+    cudaError_t e__ = (expr);                                                                    \
+    if (e__ != cudaSuccess)                                                                      \
+      return static_fail(LAYUP_ECUDA, "%s: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+  } while (0)
+
+}  // namespace
+
+extern "C" int layup_disagreement_static(const float *x_dev, int32_t K, int32_t L, const int64_t *numel,
+                                         const double *w, double *dist, void *cuda_stream) {
+  using namespace layup;
+  // ---- arguments: everything is refused before a single CUDA call is enqueued
+  if (!x_dev || !numel || !dist) return static_fail(LAYUP_EINVAL, "NULL argument");
+  if (K < 1 || K > LAYUP_MAX_K) return static_fail(LAYUP_EINVAL, "K=%d outside [1,%d]", K, LAYUP_MAX_K);
+  if (L < 1) return static_fail(LAYUP_EINVAL, "L=%d < 1", L);
+  if ((long long)L * K > LAYUP_STATIC_MAX_PAIRS)
+    return static_fail(LAYUP_EINVAL,
+                       "L*K = %lld (layer, replica) pairs exceed LAYUP_STATIC_MAX_PAIRS = %d, the size of the "
+                       "library's static scratch; use layup_disagreement (ctx-owned scratch) for this shape",
+                       (long long)L * K, LAYUP_STATIC_MAX_PAIRS);
+  if (reinterpret_cast<uintptr_t>(x_dev) % 128 != 0) return static_fail(LAYUP_EINVAL, "x_dev is not 128-byte aligned");
+  long long section = 0;                                     // floats of the X section
+  for (int l = 0; l < L; ++l) {
+    if (numel[l] < 1) return static_fail(LAYUP_EINVAL, "numel[%d]=%lld < 1", l, (long long)numel[l]);
+    section += (long long)K * ((numel[l] + 31) / 32 * 32);
+  }
+  int dev = -1;
+  STATIC_CU(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kStaticMaxDevices) return static_fail(LAYUP_EINVAL, "device ordinal %d not supported (max %d)", dev, kStaticMaxDevices - 1);
+  cudaPointerAttributes pa;
+  STATIC_CU(cudaPointerGetAttributes(&pa, x_dev));
+  if ((pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) || (pa.type == cudaMemoryTypeDevice && pa.device != dev))
+    return static_fail(LAYUP_EINVAL, "x_dev is not device memory of the current device %d", dev);
+
+  std::lock_guard<std::mutex> lock(g_static_mu);             // held to the final synchronise (layup.h "Sharing")
+  StaticDevice &sd = g_static_dev[dev];
+  if (sd.scratch == nullptr) {
+    // once per device, with that device current
+    double *ptr = nullptr;
+    STATIC_CU(cudaGetSymbolAddress(reinterpret_cast<void **>(&ptr), g_static_scratch));
+    if (ptr == nullptr) return static_fail(LAYUP_ECUDA, "cudaGetSymbolAddress returned a null address");
+    int n_sm = 0, optin = 0;
+    STATIC_CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    STATIC_CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    sd.n_sm = n_sm;
+    sd.smem_optin = (size_t)optin;
+    sd.scratch = ptr;
+  }
+  // the launch plan of layup_disagreement (function attributes + occupancy query: nothing is allocated)
+  int C = 0, stages = 0, smem = 0, ctas = 0, log2C = 0;
+  STATIC_CU(diag_plan(K, sd.smem_optin, &C, &stages, &smem, &ctas));
+  if (ctas < 1) return static_fail(LAYUP_EINVAL, "K=%d does not fit the diagnostic kernel", K);
+  while ((1 << log2C) < C) ++log2C;
+
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const size_t n = (size_t)L * K;
+  double *d_dist = sd.scratch, *d_w = sd.scratch + LAYUP_STATIC_MAX_PAIRS;
+  STATIC_CU(cudaMemsetAsync(d_dist, 0, sizeof(double) * n, s));       // last call's sums are still there
+  if (w) STATIC_CU(cudaMemcpyAsync(d_w, w, sizeof(double) * n, cudaMemcpyHostToDevice, s));
+  // work list in reverse layer order, at most kMaxPos layers per launch, as in layup_disagreement;
+  // layer offsets walked back from the end of the section (no host table is built)
+  long long end = section;
+  for (int q0 = 0; q0 < L;) {
+    PosTable tab;
+    int cnt = 0;
+    tab.prefix[0] = 0;
+    while (q0 + cnt < L && cnt < kMaxPos) {
+      const int l = L - 1 - (q0 + cnt);
+      const long long pad = (numel[l] + 31) / 32 * 32;
+      end -= (long long)K * pad;
+      tab.lay[cnt] = LayerDesc{end, pad, numel[l]};
+      tab.layer[cnt] = l;
+      tab.prefix[cnt + 1] = tab.prefix[cnt] + (pad / 4 + C - 1) / C;
+      ++cnt;
+    }
+    tab.n = cnt;
+    const long long tiles = tab.prefix[cnt];
+    const long long resident = (long long)sd.n_sm * ctas;
+    const int grid = (int)(tiles < resident ? tiles : resident);
+    STATIC_CU(launch_disagreement(x_dev, w ? d_w : nullptr, d_dist, K, C, log2C, stages, tab, grid, smem, s));
+    q0 += cnt;
+  }
+  STATIC_CU(cudaMemcpyAsync(dist, d_dist, sizeof(double) * n, cudaMemcpyDeviceToHost, s));
+  STATIC_CU(cudaStreamSynchronize(s));
+  return LAYUP_OK;
+}

@@ -95,6 +95,8 @@ struct PosTable {
   int32_t n;
 };
 
+// api.cu
+void note_error(const char *text);     // becomes the text of layup_last_error(NULL) on this host thread
 // schedule.cu
 cudaError_t launch_schedule(const SchedParams &p, int n_layers, cudaStream_t s);
 cudaError_t launch_peers_only(uint64_t seed, uint32_t step, uint32_t skip_thr, int K, int L, int peer_mode,
