@@ -93,6 +93,12 @@ def rule_kwargs(args):
     return kw
 
 
+def bench_config(w, args):
+    """The workload, identically for both arms (ours and --impl reference): what is computed, not how it is launched."""
+    return {"workload": "%s (%s)" % (w.name, w.note), "K": w.K, "L": w.L, "params_per_replica": w.params_per_replica,
+            "momentum": w.momentum, "lr": w.lr, "skip_prob": w.skip_prob, "optimizer": args.optimizer, "mix": args.mix}
+
+
 def bytes_per_update(w, args=None):
     """read x, g; write x (+ read/write m (+ read/write v))."""
     if args is not None and args.optimizer == "adamw":
@@ -112,15 +118,18 @@ def measured_peak():
 
 def committed_traffic(name, optimizer="sgd"):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture
-    (profiles/traffic.csv, see profiles/traffic.md); None if this (workload, optimizer) was not captured."""
+    (profiles/traffic.csv, see profiles/traffic.md) and where it comes from (summary file, capture date, git
+    hash of the kernels captured -- a COMMITTED figure, not a live one: a stale capture shows here);
+    (None, None) if this (workload, optimizer) was not captured."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(p):
         import csv
         with open(p) as f:
             for row in csv.DictReader(f):
                 if row["workload"] == name and row["optimizer"] == optimizer:
-                    return float(row["dram_bytes_per_launch"])
-    return None
+                    return float(row["dram_bytes_per_launch"]), "%s, captured %s at %s" % (
+                        row["source"], row.get("captured", "?"), row.get("git", "?"))
+    return None, None
 
 
 # ---- oracle sample (cpu_baseline and --impl reference) -------------------------------
@@ -131,6 +140,13 @@ def oracle_sample(w, seconds, steps=None, warmup=0, args=None, all_cores=False):
     core, bit-identical results); else the default single-threaded build."""
     import oracle
     oracle.use_omp(all_cores)
+    try:
+        return _oracle_sample(oracle, w, seconds, steps, warmup, args, all_cores)
+    finally:
+        oracle.use_omp(False)            # never leave the OpenMP build as the process-wide default
+
+
+def _oracle_sample(oracle, w, seconds, steps, warmup, args, all_cores):
     budget = 200e6                       # param-updates per round in the sample
     layers, tot = [], 0
     for l in reversed(range(w.L)):
@@ -165,7 +181,6 @@ def oracle_sample(w, seconds, steps=None, warmup=0, args=None, all_cores=False):
         elif t_used >= seconds or done >= 50:
             break
     ups = sum(per_step_updates) / t_used
-    oracle.use_omp(False)
     sample = "layers %d..%d of %d (%.1fM params/replica, K=%d), %d rounds, %s" % (
         layers[0], layers[-1], w.L, sum(sub.numel) / 1e6, sub.K, done,
         "OpenMP over elements, %d threads" % (os.cpu_count() or 1) if all_cores else "single thread")
@@ -190,8 +205,7 @@ def run_reference(args, w, rank, world):
         "metric": METRIC, "value": ups, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": s_per_step * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic", "impl": "reference",
-        "config": {"workload": "%s (%s)" % (w.name, w.note), "K": w.K, "L": w.L,
-                   "params_per_replica": w.params_per_replica, "momentum": w.momentum},
+        "config": bench_config(w, args),
         "cpu_baseline": {"value": ups, "unit": UNIT, "cores": os.cpu_count() or 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": ups, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -441,8 +455,9 @@ def run_ours(args, w, rank, world, local_rank):
         k_avg_ms, bytes_per_launch = r["ms"] / args.steps, r["bytes"] / args.steps
     achieved = bytes_per_launch / (k_avg_ms * 1e-3) / 1e9 if k_avg_ms > 0 else 0.0
     kernel = "layup_update_persist" if (tuning_dict(args) or {}).get("launch_shape") == 2 else "layup_update_tma"
+    traffic, traffic_from = committed_traffic(w.name, args.optimizer) if args.mix == "pushsum" and kernel == "layup_update_tma" else (None, None)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": committed_traffic(w.name, args.optimizer) if args.mix == "pushsum" and kernel == "layup_update_tma" else None,
+                "traffic": traffic, "traffic_from": traffic_from,
                 "kernel": kernel,
                 "kernel_ms_avg": k_avg_ms, "kernel_launches": n_k, "algorithmic_bytes_per_launch": bytes_per_launch,
                 "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0}
@@ -514,6 +529,18 @@ def run_ours(args, w, rank, world, local_rank):
     if not args.no_per_config and world == 1 and args.config == "gpt2m_k16":
         per_config = per_config_report(args, rank, local_rank, barrier, w.name, main_entry)
 
+    # the other kernels of the path, inside the object the driver's record keeps: the diagnostic's read
+    # rate and the per_config row furthest below the peak (HBM-bound rows only)
+    others = {}
+    if diag and "read_gbs" in diag:
+        others["layup_disagreement"] = {"read_gbs": diag["read_gbs"], "frac": diag["read_gbs"] / peak, "ms": diag["ms"]}
+    hbm_rows = [e for e in (per_config or []) if "effective_hbm_gbs" in e and e.get("l2", "").startswith("inputs larger")]
+    if hbm_rows:
+        worst = min(hbm_rows, key=lambda e: e["effective_hbm_gbs"])
+        others["worst_per_config_row"] = {"workload": worst["workload"], "mode": worst["mode"], "ms_per_round": worst["ms_per_round"],
+                                          "effective_hbm_gbs": worst["effective_hbm_gbs"], "frac": worst["effective_hbm_gbs"] / peak}
+    roofline["others"] = others or None
+
     if rank != 0:
         return
     cpu = None
@@ -523,10 +550,9 @@ def run_ours(args, w, rank, world, local_rank):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "%s (%s)" % (w.name, w.note), "K": w.K, "L": w.L,
-                   "params_per_replica": w.params_per_replica, "momentum": w.momentum, "lr": w.lr,
-                   "skip_prob": w.skip_prob, "mode": args.mode, "optimizer": args.optimizer, "mix": args.mix,
-                   "tuning": tuning_dict(args), "parallelism": "replicas only x%d" % world,
+        "config": bench_config(w, args),
+        # how this arm launches the workload (GPU-only settings; the reference arm has none)
+        "launch": {"mode": args.mode, "tuning": tuning_dict(args), "parallelism": "replicas only x%d" % world,
                    "l2": "inputs larger than L2" if job_bytes / args.steps / world > 4 * 126e6 else
                          "L2-resident working set (launch-latency bound, see DESIGN.md)"},
         "effective_hbm_gbs": eff_gbs, "frac_of_8TBs_nominal": eff_gbs / world / 8000.0,

@@ -11,6 +11,7 @@ registers, issue utilisation, top stall reasons) for every matching launch.
 Both read the report with `ncu -i REP --page raw --csv`; nothing here runs on a GPU.
 """
 import csv
+import os
 import io
 import re
 import subprocess
@@ -46,8 +47,15 @@ def kernel_short(name):
 
 
 def traffic(specs):
+    """Rows carry the capture date and the git hash of the kernels captured (--git HASH first: the GPU
+    box has no .git), so that bench.py can say how old the committed figure is (roofline.traffic_from)."""
+    import datetime
+    git = "?"
+    if specs and specs[0] == "--git":
+        git, specs = specs[1], specs[2:]
+    captured = datetime.date.today().isoformat()
     w = csv.writer(sys.stdout, lineterminator="\n")
-    w.writerow(["workload", "optimizer", "dram_bytes_per_launch", "kernel", "source"])
+    w.writerow(["workload", "optimizer", "dram_bytes_per_launch", "kernel", "source", "captured", "git"])
     for spec in specs:
         parts = spec.split(":")
         rep, workload, optimizer = parts[:3]
@@ -55,7 +63,45 @@ def traffic(specs):
         source = parts[4] if len(parts) > 4 else rep
         l = pick(read_raw(rep), pattern)[-1]
         total = scaled(l, "dram__bytes_read.sum") + scaled(l, "dram__bytes_write.sum")
-        w.writerow([workload, optimizer, int(round(total)), kernel_short(l["Kernel Name"][0]), source])
+        w.writerow([workload, optimizer, int(round(total)), kernel_short(l["Kernel Name"][0]), source, captured, git])
+
+
+_SASS = r"UTMALDG[.A-Z0-9_]*|UTMASTG[.A-Z0-9_]*|UBLKCP[.A-Z0-9_]*|SYNCS[.A-Z0-9_]*|LDG\.E[.A-Z0-9_]*|STG\.E[.A-Z0-9_]*|" \
+        r"LDS[.A-Z0-9_]*|STS[.A-Z0-9_]*|DFMA|DADD|DMUL|FFMA|ATOMG[.A-Z0-9_]*|RED[.A-Z0-9_]*|ACQBULK|UTCBAR|TCGEN05[.A-Z0-9_]*|HMMA[.A-Z0-9_]*"
+
+
+def sass(lib):
+    """Counts, per kernel of the built library, the SASS mnemonics that show HOW it moves data (TMA tile
+    loads UTMALDG, bulk copies UBLKCP, mbarrier ops SYNCS, plain LDG/STG, shared-memory and fp64 ops):
+    `cuobjdump -sass` read as text, no GPU needed."""
+    import subprocess
+    txt = subprocess.run(["cuobjdump", "-sass", lib], check=True, capture_output=True, text=True).stdout
+    print("# SASS instruction summary of %s (sm_100a), per kernel: static instruction counts" % os.path.basename(lib))
+    print("# command: python -m paper_2410_05985_b200.ncu_summary sass > profiles/sass_summary.txt")
+    print("# UTMALDG = TMA tensor-map tile load (.GATHER4 = tile::gather4), UBLKCP = 1-D bulk copy (cp.async.bulk),")
+    print("# SYNCS = mbarrier arrive / try_wait / expect_tx, ATOMG/RED = global atomics, DFMA/DADD = fp64 pipe")
+    name, counts, total = None, {}, 0
+
+    def flush():
+        if name is not None:
+            short = subprocess.run(["c++filt", name], capture_output=True, text=True).stdout.strip() or name
+            short = kernel_short(short)
+            body = "  ".join("%s x%d" % kv for kv in sorted(counts.items(), key=lambda kv: (-kv[1], kv[0])))
+            print("%-62s %6d instr | %s" % (short, total, body))
+
+    for line in txt.splitlines():
+        m = re.match(r"\s*Function : (\S+)", line)
+        if m:
+            flush()
+            name, counts, total = m.group(1), {}, 0
+            continue
+        m = re.match(r"\s*/\*[0-9a-f]{4,}\*/\s+(?:@!?U?P\d+\s+)?([A-Z][A-Z0-9_.]*)", line)
+        if m:
+            total += 1
+            op = m.group(1)
+            if re.fullmatch(_SASS, op):
+                counts[op] = counts.get(op, 0) + 1
+    flush()
 
 
 _SUMMARY = ["gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum",
@@ -96,6 +142,9 @@ def summary(rep, pattern):
 
 
 def main(argv):
+    if argv and argv[0] == "sass":
+        sass(argv[1] if len(argv) > 1 else os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc", "liblayup.so"))
+        return 0
     if len(argv) >= 2 and argv[0] == "traffic":
         traffic(argv[1:])
     elif len(argv) >= 2 and argv[0] == "summary":

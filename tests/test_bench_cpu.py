@@ -31,6 +31,23 @@ def test_reference_arm_prints_one_line_with_the_contract_keys():
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] == os.cpu_count()   # -fopenmp build
     assert d["e2e"]["value"] == d["value"] and d["e2e"]["h2d_bytes_per_step"] == 0
     assert "workload" in d["config"] and "model" not in d["config"]
+    # both arms print the SAME config dict (the driver's same_config check): what is computed, not how it is launched
+    import argparse
+    import bench
+    import synth
+    args = argparse.Namespace(optimizer="sgd", mix="pushsum")
+    assert d["config"] == json.loads(json.dumps(bench.bench_config(synth.workload("mlp3_k4"), args)))
+    assert sorted(d["config"]) == sorted(["workload", "K", "L", "params_per_replica", "momentum", "lr", "skip_prob",
+                                          "optimizer", "mix"])
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert src.count('"config": bench_config(w, args)') == 2          # run_reference and run_ours
+
+
+def test_committed_traffic_names_its_capture():
+    import bench
+    t, where = bench.committed_traffic("gpt2m_k16", "sgd")
+    assert t > 1e11 and "profiles/" in where and "captured 20" in where and " at " in where
+    assert bench.committed_traffic("no_such_workload") == (None, None)
 
 
 def test_reference_arm_other_ranks_stay_silent():
