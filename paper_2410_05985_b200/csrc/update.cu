@@ -13,8 +13,10 @@
 // launch shapes over the same list:
 //   grouped  : one CTA per work item; the hardware CTA scheduler drains the list in
 //              order (measured fastest on B200 for HBM-sized layers);
-//   persistent: a fixed grid of resident CTAs walks the list with a static stride
-//              (many small layers, L2-resident rounds).
+//   persistent: a fixed grid of resident CTAs walks the list with a static stride.  This LDG
+//              engine takes it only when asked for (layup_tuning.engine = 2 with launch_shape = 2)
+//              or when a launch has more than 2^31 work items; the TMA engine's persistent form
+//              is the ring kernel of update_persist.cu, which draws tiles from a ticket instead.
 #include "layup_internal.cuh"
 #include "rule.cuh"
 
