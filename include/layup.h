@@ -15,7 +15,9 @@
  *    no abort, nothing printed.  layup_last_error() gives the text of the last failure.
  *  - Pointers are HOST pointers unless the comment says DEVICE.
  *  - Launching calls (layup_layer_update, layup_round) are ASYNCHRONOUS on the given
- *    CUDA stream; device-side failures surface at layup_sync().
+ *    CUDA stream; device-side failures surface at layup_sync().  If a launching call fails
+ *    after one of its kernels was already enqueued (the schedule stage advances the device's
+ *    round counter), the ctx is POISONED: every later launching call returns LAYUP_ECUDA.
  *  - Ownership: the caller allocates the arena (device memory) and the streams and keeps
  *    them alive until layup_destroy(); the library borrows them.  It owns only its small
  *    tables (layer table, schedule tables, weights w[L][K]); it never allocates
@@ -62,7 +64,9 @@ extern "C" {
 #define LAYUP_MIX_SYMMETRIC 2 /* AD-PSGD-style pairwise averaging x_i,x_j <- (x_i+x_j)/2, ascending
                                  worker index, no push-sum weights (R23)               */
 
-#define LAYUP_MAX_K 1024  /* replicas (workers) per ctx                               */
+#define LAYUP_MAX_K 1024  /* replicas (workers) per ctx.  Accepted up to here; the kernels are tuned for
+                             the paper's worker counts and run at HBM speed for K <= 128 (>= 6.0 TB/s);
+                             K = 256 reaches 3.8-5.9 TB/s, K = 512 2.8-4.1 TB/s          */
 
 typedef struct layup_ctx layup_ctx;       /* opaque */
 typedef struct layup_graph layup_graph;   /* opaque: a captured sequence of launching calls */
@@ -96,7 +100,8 @@ typedef struct {
                            TMA load per array and tile, and in straggler mode (skip_prob > 0 or a delay
                            straggler) tile::gather4 requests of four replica rows each; 2: 1-D bulk
                            copies, one per (replica, array) row the round needs (what auto takes in
-                           straggler mode unless a row is only 128 B long, K >= 128)                */
+                           straggler mode unless a tile row is only 128 B long, i.e. 8 float4 columns:
+                           K > 64 at the default tile_items, smaller K with tile_items < 1024)      */
   int32_t stages;       /* persistent shape: depth of the TMA ring; default: as deep as fits        */
   int32_t group_threads;/* persistent shape: threads per consumer group (multiple of 32); default
                            512 with one group (768 for tiles of 2048+ items), 256 with more         */
@@ -291,8 +296,10 @@ int layup_disagreement_static(const float *x_dev, int32_t K, int32_t L, const in
  * (their `step` arguments are checked as usual and count on from the ctx's state);
  * layup_graph_end closes the capture and instantiates it; layup_graph_launch replays the
  * recorded (layer) events for whatever rounds come next, advancing the ctx's step bookkeeping
- * by what was recorded.  The learning rate in force at capture time is baked into the graph
- * (layup_set_lr needs a new capture).  Typical use: one graph = one backward's worth of
+ * by what was recorded.  Capture-time state is baked into the graph: the learning rate
+ * (layup_set_lr needs a new capture) and whether layup_trace was armed (a graph captured while
+ * tracing keeps stamping on every replay, one captured without never stamps; layup_trace calls
+ * after the capture do not change either).  Typical use: one graph = one backward's worth of
  * per-layer events, or one or several whole rounds of an L2-resident model, where the launch
  * overhead, not HBM, is the cost.  layup_sync checks the device counters against
  * the host's bookkeeping (LAYUP_ESTATE on disagreement). */

@@ -57,7 +57,7 @@ struct layup_ctx {
   long long fused_max_tiles = 0;          // ... and is taken by launches of at most this many work items
   unsigned char *d_active_scratch = nullptr;
   uint32_t *d_step = nullptr;             // [L] round each layer runs next (device state, see layup.h graphs)
-  int32_t *d_ps_ticket = nullptr;         // [n_ps_ticket] tile tickets of persistent update launches
+  int32_t *d_ps_ticket = nullptr;         // [L] tile tickets of persistent update launches, by work-list position
   int n_ps_ticket = 0;
   unsigned long long *d_trace = nullptr;  // [L] layup_trace
   bool tracing = false;
@@ -344,7 +344,7 @@ extern "C" int layup_init(const layup_config *cfg, void *arena_dev, size_t arena
   CU_TRY_INIT(cudaMalloc(&ctx->d_dist, sizeof(double) * L * K));
   CU_TRY_INIT(cudaMalloc(&ctx->d_step, sizeof(uint32_t) * L));
   CU_TRY_INIT(cudaMemset(ctx->d_step, 0, sizeof(uint32_t) * L));
-  ctx->n_ps_ticket = (L + kMaxPos - 1) / kMaxPos + 8;
+  ctx->n_ps_ticket = L;                   // one per work-list position: launches on different streams never share one
   CU_TRY_INIT(cudaMalloc(&ctx->d_ps_ticket, sizeof(int32_t) * ctx->n_ps_ticket));
   CU_TRY_INIT(cudaMemset(ctx->d_ps_ticket, 0, sizeof(int32_t) * ctx->n_ps_ticket));
   CU_TRY_INIT(cudaMalloc(&ctx->d_trace, sizeof(unsigned long long) * L));
@@ -494,7 +494,11 @@ static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_
   sp.ticket = ctx->d_ticket;
   sp.ps_ticket = ctx->d_ps_ticket; sp.n_ps_ticket = ctx->ps_ok ? ctx->n_ps_ticket : 0;
   const bool fused = ctx->fused_ok && ctx->tile_prefix[pos_end] - ctx->tile_prefix[pos_begin] <= ctx->fused_max_tiles;
-  if (!fused) CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
+  *n_kernels = 0;                                     // kernels enqueued so far (the caller poisons the ctx on a late failure)
+  if (!fused) {
+    CU_TRY(ctx, launch_schedule(sp, pos_end - pos_begin, s));
+    *n_kernels += 1;
+  }
 
   UpdateParams up{};
   up.x = ctx->arena;
@@ -535,8 +539,7 @@ static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_
       tab.n = n;
       // only the first update launch directly follows the schedule kernel on the stream
       if (ctx->ps_ok && !fused) {
-        if (n_launch >= ctx->n_ps_ticket) return fail(ctx, LAYUP_EINVAL, "round needs more than %d persistent launches", ctx->n_ps_ticket);
-        up.ps_ticket = ctx->d_ps_ticket + n_launch;
+        up.ps_ticket = ctx->d_ps_ticket + q0;          // the slot of this launch's first position (schedule.cu re-arms it)
         const int grid = (int)std::min<long long>(tab.prefix[n], (long long)ctx->n_sm * ctx->ps_ctas);
         CU_TRY(ctx, launch_update_persist(up, tab, grid, ctx->ps_smem, ctx->ps_stages, ctx->ps_groups, ctx->ps_gs, ctx->pdl && n_launch == 0, s));
       } else {
@@ -546,15 +549,15 @@ static int issue_kernels(layup_ctx *ctx, int pos_begin, int pos_end, cudaStream_
       }
       q0 += n;
       ++n_launch;
+      *n_kernels += 1;
     }
   } else {
     // LDG kernel: grouped (one CTA per work item) unless a persistent grid was asked for
     const bool persistent = ctx->persistent || tiles > 0x7FFFFFFFll;
     const int grid = (int)(persistent ? std::min<long long>(tiles, resident) : tiles);
     CU_TRY(ctx, launch_update(up, ctx->variant, persistent, grid, ctx->smem, s));
-    n_launch = 1;
+    *n_kernels += 1;
   }
-  *n_kernels = (fused ? 0 : 1) + n_launch;
   return LAYUP_OK;
 }
 
@@ -578,7 +581,12 @@ static int issue(layup_ctx *ctx, int64_t step, int pos_begin, int pos_end, cudaS
   if (rc == LAYUP_OK) rc = issue_kernels(ctx, pos_begin, pos_end, s, &n_kernels);
   if (rc == LAYUP_OK && prof && cudaEventRecord(ev.second, s) != cudaSuccess) rc = fail(ctx, LAYUP_ECUDA, "cudaEventRecord failed");
   if (prof) (rc == LAYUP_OK ? ctx->prof_pending : ctx->prof_pool).push_back(ev);   // never leaked
-  if (rc != LAYUP_OK) return rc;
+  if (rc != LAYUP_OK) {
+    // a kernel of this call is already on the stream (the schedule stage advances the device's round
+    // counter and halves the weights): the host's bookkeeping can no longer be trusted to match
+    if (n_kernels > 0 && !ctx->capturing) ctx->poisoned = true;
+    return rc;
+  }
   ctx->launches += n_kernels;
   for (int p = pos_begin; p < pos_end; ++p) {
     ctx->last_order.push_back(ctx->L - 1 - p);

@@ -50,8 +50,8 @@ struct SchedParams {
   double *bpow;             // [L*K*2] (beta1^t, beta2^t) per (layer, replica), AdamW only
   double lr, beta1, beta2;  // fp32 values widened
   int32_t *ticket;          // [L] zero between launches; fused single-launch path only (update_tma.cu)
-  int32_t *ps_ticket;       // [n_ps_ticket] tile tickets of the persistent update launches behind this schedule
-  int32_t n_ps_ticket;      //   kernel (update_persist.cu); zeroed here
+  int32_t *ps_ticket;       // [L] tile tickets of persistent update launches (update_persist.cu), by work-list
+  int32_t n_ps_ticket;      //   position; the schedule kernel zeroes the slots of its own layers; 0 = none
 };
 constexpr int kFusedMaxK = 64;         // the in-kernel schedule stage is O(K) per thread
 
@@ -94,6 +94,22 @@ struct PosTable {
   int32_t layer[kMaxPos];
   int32_t n;
 };
+
+// The dynamic shared memory a kernel may be launched with is an attribute of the FUNCTION on the device,
+// shared by every ctx of the process: a ctx that set it to its own (smaller) need would break the launches
+// of an older ctx that needs more (two LayUp objects alive at once: "invalid argument" at launch).  So the
+// library always opens a kernel up to the device's opt-in maximum; a launch still gets what it asks for.
+inline cudaError_t allow_max_dynamic_smem(const void *fn, int need_bytes) {
+  int dev = 0, optin = 0;
+  cudaFuncAttributes fa;
+  cudaError_t e;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  if ((e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev)) != cudaSuccess) return e;
+  if ((e = cudaFuncGetAttributes(&fa, fn)) != cudaSuccess) return e;
+  const int most = optin - (int)fa.sharedSizeBytes;
+  if (need_bytes > most) return cudaErrorInvalidValue;
+  return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, most);
+}
 
 // api.cu
 void note_error(const char *text);     // becomes the text of layup_last_error(NULL) on this host thread

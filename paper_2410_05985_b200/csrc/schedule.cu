@@ -24,8 +24,10 @@ __global__ void __launch_bounds__(1024) layup_schedule_kernel(const SchedParams 
   // the update kernel behind this one on the stream may start now (it waits for this grid's
   // completion with griddepcontrol.wait before it reads the tables)
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  if (blockIdx.x == 0)                                           // tile tickets of the persistent update launches
-    for (int t = threadIdx.x; t < p.n_ps_ticket; t += blockDim.x) p.ps_ticket[t] = 0;
+  // tile tickets of the persistent update launches behind this kernel: one slot per work-list position
+  // (position q = layer L-1-q; a launch draws from the slot of its FIRST position).  Only the slots of
+  // this call's own layers are re-armed, so per-layer events on other streams keep theirs.
+  if (p.n_ps_ticket > 0 && threadIdx.x == 0) p.ps_ticket[p.L - 1 - (p.layer_begin + (int)blockIdx.x)] = 0;
   schedule_layer(p, p.layer_begin + blockIdx.x, sm);
 }
 

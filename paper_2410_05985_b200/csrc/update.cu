@@ -218,7 +218,7 @@ cudaError_t update_kernel_setup(int variant, int opt, bool symmetric, int smem_b
   cudaError_t e;
   const int sym = symmetric ? 1 : 0;
   for (KernelFn f : {v.grouped[opt][sym], v.persistent[opt][sym]}) {
-    if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
+    if ((e = allow_max_dynamic_smem((const void *)f, smem_bytes)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
   }
   int a = 0;

@@ -331,7 +331,7 @@ cudaError_t persist_kernel_setup(int opt, bool symmetric, int smem_bytes, int *c
   if (opt < 0 || opt > 2) return cudaErrorInvalidValue;
   cudaError_t e;
   PsFn f = kPs[opt][symmetric ? 1 : 0];
-  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
+  if ((e = allow_max_dynamic_smem((const void *)f, smem_bytes)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, f, kPsMaxThreads, smem_bytes);
 }

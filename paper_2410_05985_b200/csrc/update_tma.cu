@@ -488,7 +488,7 @@ cudaError_t tma_kernel_setup(int variant, int opt, bool symmetric, bool strag, i
   int occ = 1 << 30;
   for (TmaFn f : {v.fn[strag ? 1 : 0][opt][symmetric ? 1 : 0], v.fused[strag ? 1 : 0][opt][symmetric ? 1 : 0]}) {
     if (!f) continue;
-    if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)) != cudaSuccess) return e;
+    if ((e = allow_max_dynamic_smem((const void *)f, smem_bytes)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
     int a = 0;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, f, v.threads, smem_bytes)) != cudaSuccess) return e;
