@@ -198,6 +198,157 @@ __global__ void __launch_bounds__(NCW * 32 + 32 * kDiagProducers, 1)
   flush(pos);
 }
 
+// ---- split form (32 < K <= 64): eight lane groups of a warp share the warp's 16 columns.
+// Lane l = (g, jj), g = l / 4, jj = l % 4, owns the four columns 4jj .. 4jj+3 of the warp's block (one
+// float4) for the RPL = KT/8 replicas g*RPL .. g*RPL + RPL-1: one LDS.128 per replica.  The values
+// stay in registers as fp32 (4*RPL registers), so the stage is handed back right after the loads --
+// the whole ring is in flight, none of it parked under the two passes -- and the K accumulators of a
+// column are spread over eight lanes (RPL fp64 registers each instead of KT), which leaves room for
+// a tile row of only 128 floats: 32 KB stages at K = 64, six deep, where the one-column-per-thread
+// form has three of 64 KB.  The partial consensus sums of the eight groups meet through three
+// __shfl_xor_sync steps; no shared-memory exchange and no barrier besides the ring's mbarriers.
+// (The two groups of a quarter-warp read the same 16 banks in different rows, a two-way conflict:
+// shared memory then moves 64 B per clock per SM, still three times what HBM feeds an SM.)
+// Slice pads are multiples of 32 floats, so a warp's 16-column block of a ragged last tile is
+// either wholly inside the slice or wholly outside.
+
+// fp32 -> fp64 of a value that was widened once already: `volatile` keeps the compiler from carrying the
+// first pass's doubles (twice the registers of the fp32 tile) across to the second pass
+__device__ __forceinline__ double widen_again(float f) {
+  double d;
+  asm volatile("cvt.f64.f32 %0, %1;" : "=d"(d) : "f"(f));
+  return d;
+}
+__device__ __forceinline__ double shfl_add(double v, int mask) { return v + __shfl_xor_sync(0xFFFFFFFFu, v, mask); }
+
+template <int KT, int NCW>
+__global__ void __launch_bounds__(NCW * 32 + 32 * kDiagProducers, 1)
+    layup_disagreement_split(const __grid_constant__ DiagParams p, const __grid_constant__ PosTable tab) {
+  static_assert(KT % 8 == 0, "eight lane groups share the replicas");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int NC = NCW * 32;                                           // consumer threads
+  constexpr int TF = NCW * 16;                                           // floats per replica row of a tile
+  constexpr int RPL = KT / 8;                                            // replicas per lane
+  const int K = p.K, S = p.stages, tid = threadIdx.x;
+  float *ring = reinterpret_cast<float *>(smem_raw);                    // [S][K][TF]
+  uint64_t *full = reinterpret_cast<uint64_t *>(ring + (size_t)S * K * TF);   // [S]
+  uint64_t *empty = full + S;                                           // [S]
+  double *coef_all = reinterpret_cast<double *>(empty + S);             // [consumer warps][KT]
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) {
+      mbar_init(full + s, 1);
+      mbar_init(empty + s, NCW);
+    }
+  }
+  __syncthreads();
+
+  const long long n_tiles = tab.prefix[tab.n];
+  const long long t0 = n_tiles * blockIdx.x / gridDim.x, t1 = n_tiles * (blockIdx.x + 1) / gridDim.x;
+  if (t0 >= t1) return;
+  int pos = 0;
+  {
+    int lo = 0, hi = tab.n;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (t0 >= tab.prefix[mid]) lo = mid; else hi = mid;
+    }
+    pos = lo;
+  }
+
+  if (tid >= NC) {
+    // ---------------- producer warps: as in the ring kernel above
+    const int lane = (tid - NC) & 31, pw = (tid - NC) >> 5;
+    int s = 0;
+    uint32_t ph = 0;
+    for (long long tile = t0; tile < t1; ++tile) {
+      while (tile >= tab.prefix[pos + 1]) ++pos;
+      const long long pad = tab.lay[pos].pad;
+      const long long f0 = (tile - tab.prefix[pos]) * TF;
+      const long long left = pad - f0;
+      const uint32_t chunk = (uint32_t)(left < TF ? left : TF) * 4u;     // multiple of 128 B
+      const float *src = p.x + tab.lay[pos].base + f0;
+      mbar_wait(empty + s, ph ^ 1u);
+      if (lane == 0 && pw == 0) mbar_expect_tx(full + s, chunk * (uint32_t)K);
+      __syncwarp();
+      float *dst = ring + (size_t)s * K * TF;
+      for (int i = pw + kDiagProducers * lane; i < K; i += 32 * kDiagProducers)
+        bulk_g2s(dst + (size_t)i * TF, src + (long long)i * pad, chunk, full + s);
+      if (++s == S) { s = 0; ph ^= 1u; }
+    }
+    return;
+  }
+
+  // ---------------- consumers
+  const int lane = tid & 31, g = lane >> 2, jj = lane & 3;
+  const int wc0 = (tid >> 5) * 16;                                      // first column of this warp's block
+  const int r0 = g * RPL;                                               // first replica of this lane group
+  double acc[RPL];
+#pragma unroll
+  for (int k = 0; k < RPL; ++k) acc[k] = 0.0;
+  const double inv_k = 1.0 / (double)K;
+  double *coef = coef_all + (size_t)(tid >> 5) * KT;
+  auto load_coef = [&](int qpos) {                                      // plain mean: the scalar 1/K, stored all the same
+    __syncwarp();
+    for (int i = lane; i < KT; i += 32)
+      coef[i] = i < K ? (p.w != nullptr ? __ldg(p.w + (size_t)tab.layer[qpos] * K + i) : inv_k) : 0.0;
+    __syncwarp();
+  };
+  auto flush = [&](int qpos) {
+#pragma unroll
+    for (int k = 0; k < RPL; ++k) {
+      const double v = shfl_add(shfl_add(acc[k], 1), 2);                // the four lanes of a group: 16 columns
+      if (jj == 0 && r0 + k < K) atomicAdd(p.dist + (size_t)tab.layer[qpos] * K + r0 + k, v);
+      acc[k] = 0.0;
+    }
+  };
+  load_coef(pos);
+  int s = 0;
+  uint32_t ph = 0;
+  for (long long tile = t0; tile < t1; ++tile) {
+    if (tile >= tab.prefix[pos + 1]) {
+      flush(pos);
+      while (tile >= tab.prefix[pos + 1]) ++pos;
+      load_coef(pos);
+    }
+    const long long left = tab.lay[pos].pad - (tile - tab.prefix[pos]) * TF;
+    const bool live = wc0 < left;                                       // warp-uniform: `left` is a multiple of 32
+    const float *rows = ring + (size_t)s * K * TF + (size_t)r0 * TF + wc0 + 4 * jj;
+    float4 xf[RPL];
+    mbar_wait(full + s, ph);
+    if (live) {
+#pragma unroll
+      for (int k = 0; k < RPL; ++k)
+        xf[k] = (KT == K || r0 + k < K) ? *reinterpret_cast<const float4 *>(rows + (size_t)k * TF)
+                                        : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty + s);                              // the tile now lives in registers
+    if (live) {
+      double m[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+      for (int k = 0; k < RPL; ++k) {
+        const double c = coef[r0 + k];                                  // 0 for replicas beyond K
+        m[0] = fma(c, (double)xf[k].x, m[0]); m[1] = fma(c, (double)xf[k].y, m[1]);
+        m[2] = fma(c, (double)xf[k].z, m[2]); m[3] = fma(c, (double)xf[k].w, m[3]);
+      }
+#pragma unroll
+      for (int v = 0; v < 4; ++v) m[v] = shfl_add(shfl_add(shfl_add(m[v], 4), 8), 16);   // lanes with the same jj
+#pragma unroll
+      for (int k = 0; k < RPL; ++k) {
+        if (KT == K || r0 + k < K) {
+          double d;
+          d = widen_again(xf[k].x) - m[0]; acc[k] = fma(d, d, acc[k]);
+          d = widen_again(xf[k].y) - m[1]; acc[k] = fma(d, d, acc[k]);
+          d = widen_again(xf[k].z) - m[2]; acc[k] = fma(d, d, acc[k]);
+          d = widen_again(xf[k].w) - m[3]; acc[k] = fma(d, d, acc[k]);
+        }
+      }
+    }
+    if (++s == S) { s = 0; ph ^= 1u; }
+  }
+  flush(pos);
+}
+
 // ---- general form (K > 64): consensus of every column through shared memory, one or two stages
 constexpr int kGenThreads = 256;
 template <int MAXIT>
@@ -325,7 +476,9 @@ struct RingShape {
   int kt, ncw, cpt;     // a tile row is ncw * 32 * cpt floats
   DiagFn fn;
   bool exact;           // only for K == kt (its predicated path would be slower than a general shape's)
+  int tf = 0;           // floats per tile row if not ncw * 32 * cpt (split form: ncw * 16)
 };
+int ring_tf(const RingShape *r) { return r->tf ? r->tf : r->ncw * 32 * r->cpt; }
 // one CTA per SM: the registers go to the per-replica accumulators (and the fp64 copy of the tile),
 // the shared memory to a deep ring; 16 consumer warps while the accumulators allow it (8 were measured
 // issue-bound: profiles/r2_disagreement_gpt2m_k16_8warps.txt)
@@ -335,14 +488,15 @@ struct RingShape {
 #define LAYUP_DIAG(KT_, CPT_) {KT_, 16, CPT_, layup_disagreement_kernel<KT_, true, 16, CPT_>, false}
 // 16 < K <= 32: the converted tile still fits in registers with 8 consumer warps (K = 32: 6.2 -> 6.8 TB/s)
 #define LAYUP_DIAG8(KT_, KEEP_) {KT_, 8, 1, layup_disagreement_kernel<KT_, KEEP_, 8>, true}
+#define LAYUP_DIAGQ(KT_) {KT_, 8, 1, layup_disagreement_split<KT_, 8>, false, 8 * 16}
 const RingShape kRing[] = {
     LAYUP_DIAG(1, 8),  LAYUP_DIAG(2, 8),  LAYUP_DIAG(3, 4),  LAYUP_DIAG(4, 4),  LAYUP_DIAG(5, 3),  LAYUP_DIAG(6, 2),
     LAYUP_DIAG(7, 2),  LAYUP_DIAG(8, 2),  LAYUP_DIAG(9, 1),  LAYUP_DIAG(10, 1), LAYUP_DIAG(11, 1), LAYUP_DIAG(12, 1),
     LAYUP_DIAG(13, 1), LAYUP_DIAG(14, 1), LAYUP_DIAG(15, 1), LAYUP_DIAG(16, 1),
     LAYUP_DIAG8(20, true), LAYUP_DIAG8(24, true), LAYUP_DIAG8(28, true), LAYUP_DIAG8(32, true),
-    LAYUP_DIAG8(40, false), LAYUP_DIAG8(48, false), LAYUP_DIAG8(56, false),
     {32, 16, 1, layup_disagreement_kernel<32, false, 16>, false},
-    {64, 8, 1, layup_disagreement_kernel<64, false, 8>, false},
+    // 32 < K <= 64: the split form (eight lane groups share a 16-column block, tile in fp32 registers, 128-float rows)
+    LAYUP_DIAGQ(40), LAYUP_DIAGQ(48), LAYUP_DIAGQ(56), LAYUP_DIAGQ(64),
 };
 const RingShape *ring_shape(int K) {
   for (const RingShape &r : kRing)
@@ -366,7 +520,7 @@ int general_iters(int K, int C) { return (K * C + kGenThreads - 1) / kGenThreads
 cudaError_t diag_plan(int K, size_t smem_optin, int *C, int *stages, int *smem_bytes, int *ctas_per_sm) {
   cudaError_t e;
   if (const RingShape *r = ring_shape(K)) {
-    const int tf = r->ncw * 32 * r->cpt;
+    const int tf = ring_tf(r);
     // as deep as fits in the ~224 KB of shared memory of the SM's one CTA
     const size_t budget = (size_t)(224 * 1024) - 1024 - sizeof(double) * r->ncw * r->kt;
     int S = (int)((budget < smem_optin ? budget : smem_optin) / ((size_t)K * tf * sizeof(float) + 16));
@@ -375,7 +529,7 @@ cudaError_t diag_plan(int K, size_t smem_optin, int *C, int *stages, int *smem_b
       *C = tf / 4;
       *stages = S;
       *smem_bytes = (int)ring_smem(K, tf, S, r->kt, r->ncw);
-      if ((e = cudaFuncSetAttribute(r->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, *smem_bytes)) != cudaSuccess) return e;
+      if ((e = allow_max_dynamic_smem((const void *)r->fn, *smem_bytes)) != cudaSuccess) return e;
       if ((e = cudaFuncSetAttribute(r->fn, cudaFuncAttributePreferredSharedMemoryCarveout, 100)) != cudaSuccess) return e;
       return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, r->fn, r->ncw * 32 + 32 * kDiagProducers, *smem_bytes);
     }
@@ -388,7 +542,7 @@ cudaError_t diag_plan(int K, size_t smem_optin, int *C, int *stages, int *smem_b
   *smem_bytes = (int)general_smem(K, c, two);
   if (general_iters(K, c) > 32) return cudaErrorInvalidValue;
   auto f = general_iters(K, c) <= 8 ? layup_disagreement_general<8> : layup_disagreement_general<32>;
-  if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, *smem_bytes)) != cudaSuccess) return e;
+  if ((e = allow_max_dynamic_smem((const void *)f, *smem_bytes)) != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, f, kGenThreads, *smem_bytes);
 }
 
@@ -396,7 +550,7 @@ cudaError_t launch_disagreement(const float *x, const double *w, double *dist, i
                                 const PosTable &tab, int grid, int smem_bytes, cudaStream_t s) {
   DiagParams p{x, w, dist, K, C, log2C, stages};
   const RingShape *r = ring_shape(K);
-  if (r && C * 4 == r->ncw * 32 * r->cpt && stages >= 2 && (size_t)smem_bytes == ring_smem(K, C * 4, stages, r->kt, r->ncw)) {
+  if (r && C * 4 == ring_tf(r) && stages >= 2 && (size_t)smem_bytes == ring_smem(K, C * 4, stages, r->kt, r->ncw)) {
     r->fn<<<grid, r->ncw * 32 + 32 * kDiagProducers, smem_bytes, s>>>(p, tab);
     return cudaGetLastError();
   }

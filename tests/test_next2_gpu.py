@@ -41,7 +41,8 @@ def test_delay_mode_parity(K, r, n, p):
     lu.close()
 
 
-@pytest.mark.parametrize("K", [1, 2, 3, 8, 16, 64, 200, 1000])
+# 33 ... 63: the split form of the ring kernel (eight lane groups per column block), exact and predicated K
+@pytest.mark.parametrize("K", [1, 2, 3, 8, 16, 33, 40, 47, 48, 56, 63, 64, 200, 1000])
 def test_disagreement_parity(K):
     numel = [1, 33, 1000, 4097, 70001 if K <= 16 else 2049]
     w = synth.Workload("dis", K, tuple(numel), lr=0.05, momentum=0.0, rounds=3, seed=5 + K, grad_std=1e-2)
@@ -101,4 +102,31 @@ def test_disagreement_full_size_and_bandwidth():
     gbs = 4.0 * w.K * w.params_per_replica / dt / 1e9
     print("layup_disagreement on configs[2]: %.3f ms per call on the device, %.0f GB/s read" % (dt * 1e3, gbs))
     assert gbs > 4500
+    lu.close()
+
+
+def test_disagreement_bandwidth_k64():
+    """configs[4] shapes (K = 64, 40 layers of 4 K ... 1 M elements): the split form's read rate, and its
+    distances against the oracle on every layer."""
+    w = synth.workload("manysmall_k64")
+    lu = LayUp(w.K, w.numel, w.lr, w.momentum, w.seed)
+    for l in range(w.L):
+        synth.fill_init_(w, l, lu.view(WHAT_X, l))
+        synth.fill_grad_(w, 0, l, lu.view(WHAT_G, l))
+    lu.layup_round(0)
+    lu.layup_sync()
+    wts = lu.layup_weights()
+    for weighted in (False, True):
+        got = lu.layup_disagreement(weighted)
+        for l in range(w.L):
+            want = oracle.disagreement(lu.view(WHAT_X, l).cpu().numpy(), wts[l] if weighted else None)
+            assert np.abs(got[l] - want).max() <= 1e-9 * want.max(), (l, weighted)
+    ms = []
+    for _ in range(9):
+        lu.layup_disagreement(False)
+        ms.append(lu.layup_disagreement_ms())
+    dt = float(np.median(ms)) * 1e-3
+    gbs = 4.0 * w.K * w.params_per_replica / dt / 1e9
+    print("layup_disagreement on configs[4]: %.3f ms per call on the device, %.0f GB/s read" % (dt * 1e3, gbs))
+    assert gbs > 4800            # measured 5370 (round 2's one-column-per-thread form: 4300)
     lu.close()
