@@ -127,3 +127,40 @@ def test_header_is_plain_c(tmp_path):
                    '  return layup_arena_bytes(&c, &n) == LAYUP_EINVAL ? (int)sizeof(c) : -1; }\n')
     subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"),
                            "-c", str(src), "-o", str(tmp_path / "use_layup.o")])
+
+
+def _cc(tmp_path, defines, libs):
+    exe = str(tmp_path / ("c_abi" + ("_layout" if defines else "")))
+    cuda = os.environ.get("CUDA_HOME", "/usr/local/cuda")
+    csrc = os.path.join(ROOT, "paper_2410_05985_b200", "csrc")
+    cmd = ["gcc", "-std=gnu99", "-Wall", "-Werror", "-I" + os.path.join(ROOT, "include"), "-I" + os.path.join(cuda, "include")] + \
+          defines + [os.path.join(ROOT, "tests", "c_abi_driver.c"), "-o", exe]
+    if libs:
+        cmd += ["-L" + csrc, "-llayup", "-L" + os.path.join(cuda, "lib64"), "-lcudart",
+                "-Wl,-rpath," + csrc, "-Wl,-rpath," + os.path.join(cuda, "lib64")]
+    import subprocess
+    subprocess.check_call(cmd)
+    return exe
+
+
+def test_struct_layout_seen_by_a_c_compiler_matches_the_ctypes_mirror(tmp_path):
+    """sizeof / offsetof of layup_config and layup_tuning as gcc lays them out (tests/c_abi_driver.c
+    -DLAYOUT_ONLY) against binding._Config / _Tuning: the Python mirror is hand-written."""
+    import subprocess
+    out = subprocess.run([_cc(tmp_path, ["-DLAYOUT_ONLY"], False)], capture_output=True, text=True, check=True).stdout
+    got = dict(line.split() for line in out.splitlines())
+    assert int(got.pop("sizeof.layup_config")) == ctypes.sizeof(binding._Config)
+    assert int(got.pop("sizeof.layup_tuning")) == ctypes.sizeof(binding._Tuning)
+    want = {"layup_config.%s" % n: getattr(binding._Config, n).offset for n, _ in binding._Config._fields_}
+    want.update({"layup_tuning.%s" % n: getattr(binding._Tuning, n).offset for n, _ in binding._Tuning._fields_})
+    assert {k: int(v) for k, v in got.items()} == want
+
+
+def test_c_program_links_against_the_library(lib, tmp_path):
+    """The compute half of tests/c_abi_driver.c builds and links against liblayup.so here; it RUNS in
+    tests/test_zy_c_abi_gpu.py on the GPU box.  Without a device it must fail loudly, not fall back."""
+    import subprocess
+    exe = _cc(tmp_path, [], True)
+    if not torch.cuda.is_available():
+        r = subprocess.run([exe], capture_output=True, text=True)
+        assert r.returncode != 0 and "C_ABI_OK" not in r.stdout
